@@ -1,0 +1,304 @@
+/*
+ * d2sd_oracle.c -- CPU oracle for the D2SD verification hot path.
+ *
+ * TEST INFRASTRUCTURE, NOT PRODUCT.  Only tests/, __graft_entry__.smoke() and bench.py's
+ * cpu_baseline / --impl reference legs may load this library.  It shares no code, header,
+ * table or helper with the CUDA path under paper_2606_04446_b200/ and neither imports the other.
+ *
+ * Plain, slow, obviously-correct C written from /root/reference/PAPER.md (arXiv 2606.04446) and,
+ * where the paper is silent or garbled, from the readings G1..G21 listed in DESIGN.md.
+ * Floating point is fp64 throughout; bf16 inputs are widened exactly.  No blocking, fusion or
+ * re-association: attention is the explicit full masked softmax per (node, head); selection is a
+ * full ranking; the mask is built by parent chasing; acceptance is the path walk.  The only
+ * parallelism is an OpenMP "for" over independent output items.
+ *
+ * Pins (tests/test_oracle_pins.py, all run under -m "not gpu"):
+ *   select : P1 telescoping closed form, P2 special cases + exhaustive grids vs an independent sort
+ *   build  : P3 brute force over the K+1 flat candidate sequences, P4 structural invariants
+ *   attn   : P3 (flat-sequence causal attention), P5 merge invariant, P6 torch SDPA fp64 special case
+ *   accept : P7 special cases, P8 per-candidate linear rule, P9 numpy.argmax + planted ties
+ * Parity unpinned: none of the functions below.  (alpha / speedup tables of the paper are not
+ * computed here at all: they need weights and datasets.)
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+/* bf16 bit pattern -> double, exact. */
+static double bf16_to_f64(uint16_t b) {
+    uint32_t u = ((uint32_t)b) << 16;
+    float f;
+    memcpy(&f, &u, sizeof f);
+    return (double)f;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Stage (a): rejection-boundary posterior and top-K prefix selection.
+ * PAPER.md:87-97 Eq. 3-4: r(i) = (prod_{k=1..i} c_k) * (1 - c_{i+1}),  i = 0..gamma-2   [G1]
+ * PAPER.md:103-105 Eq. 5: S = Top-K_i r(i) over i in {0..gamma-2}                       [G2-G4]
+ * Readings: fp32 confidences widened to fp64; sequential left-to-right product, one subtract and
+ * one multiply per r(i), no FMA [G7]; ties -> smaller i [G5]; S emitted ascending [G6];
+ * conf[.,0] (anchor slot) ignored [G9].
+ * conf [B,gamma] -> prefix_len [B,K]; r_out [B,gamma-1] optional.
+ * ------------------------------------------------------------------------------------------ */
+void d2sd_oracle_select(const float* conf, int32_t B, int32_t gamma, int32_t K,
+                        int32_t* prefix_len, double* r_out) {
+    int32_t n = gamma - 1;
+    double* r = (double*)malloc(sizeof(double) * (size_t)(n > 0 ? n : 1));
+    int32_t* order = (int32_t*)malloc(sizeof(int32_t) * (size_t)(n > 0 ? n : 1));
+    for (int32_t b = 0; b < B; ++b) {
+        const float* c = conf + (size_t)b * gamma;
+        volatile double P = 1.0; /* volatile: forbid contraction/reordering of the stated order */
+        for (int32_t i = 0; i < n; ++i) {
+            volatile double one_minus = 1.0 - (double)c[i + 1];
+            volatile double ri = P * one_minus;
+            r[i] = ri;
+            volatile double Pn = P * (double)c[i + 1];
+            P = Pn;
+        }
+        if (r_out) memcpy(r_out + (size_t)b * n, r, sizeof(double) * (size_t)n);
+        /* full ranking by (r descending, i ascending): stable insertion sort */
+        for (int32_t i = 0; i < n; ++i) order[i] = i;
+        for (int32_t i = 1; i < n; ++i) {
+            int32_t x = order[i];
+            int32_t j = i - 1;
+            while (j >= 0 && r[order[j]] < r[x]) { order[j + 1] = order[j]; --j; }
+            order[j + 1] = x;
+        }
+        /* first K of the ranking, emitted ascending in i */
+        int32_t* out = prefix_len + (size_t)b * K;
+        for (int32_t k = 0; k < K; ++k) out[k] = order[k];
+        for (int32_t i = 1; i < K; ++i) {
+            int32_t x = out[i];
+            int32_t j = i - 1;
+            while (j >= 0 && out[j] > x) { out[j + 1] = out[j]; --j; }
+            out[j + 1] = x;
+        }
+    }
+    free(r);
+    free(order);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Stage (b): shared-prefix tree.
+ * branch i keeps the anchor and the first i draft-1 tokens and re-drafts
+ * positions i+1..gamma-1; it shares its first i+1 tokens with draft 1.  Flattened-tree layout is
+ * BASELINE.json's; node order / mask packing per [G12-G14]: trunk nodes 0..gamma-1 first, then
+ * branches in ascending prefix length; pos_id = ctx_len + depth; uint32 mask words, bit (a%32)
+ * of word a/32, self bit set; padding rows get tokens/parent = -1, depth/pos = 0, mask = 0.
+ * The mask is built by PARENT CHASING (row n = row parent[n] plus bit n).
+ * ------------------------------------------------------------------------------------------ */
+void d2sd_oracle_build_tree(const int32_t* draft1, const int32_t* draft2, const int32_t* prefix_len,
+                            const int32_t* ctx_len, int32_t B, int32_t gamma, int32_t K,
+                            int32_t T_cap, int32_t* tokens, int32_t* parent, int32_t* depth,
+                            int32_t* pos_id, int32_t* branch_off, uint32_t* mask,
+                            int32_t* tree_len) {
+    int32_t W = (T_cap + 31) / 32;
+    for (int32_t b = 0; b < B; ++b) {
+        int32_t* tok = tokens + (size_t)b * T_cap;
+        int32_t* par = parent + (size_t)b * T_cap;
+        int32_t* dep = depth + (size_t)b * T_cap;
+        int32_t* pos = pos_id + (size_t)b * T_cap;
+        uint32_t* mk = mask + (size_t)b * T_cap * W;
+        int32_t* boff = branch_off + (size_t)b * (K + 1);
+        for (int32_t n = 0; n < T_cap; ++n) { tok[n] = -1; par[n] = -1; dep[n] = 0; pos[n] = 0; }
+        memset(mk, 0, sizeof(uint32_t) * (size_t)T_cap * W);
+        /* trunk = draft-1 block (position 0 = anchor, root of the tree [G10]) */
+        for (int32_t j = 0; j < gamma; ++j) {
+            tok[j] = draft1[(size_t)b * gamma + j];
+            par[j] = j - 1;
+            dep[j] = j;
+        }
+        int32_t off = gamma;
+        for (int32_t k = 0; k < K; ++k) {
+            int32_t i = prefix_len[(size_t)b * K + k];
+            boff[k] = off;
+            for (int32_t p = i + 1; p <= gamma - 1; ++p) {
+                int32_t n = off + (p - i - 1);
+                tok[n] = draft2[((size_t)b * K + k) * gamma + p];
+                par[n] = (p == i + 1) ? i : n - 1;
+                dep[n] = p;
+            }
+            off += gamma - 1 - i;
+        }
+        boff[K] = off;
+        tree_len[b] = off;
+        for (int32_t n = 0; n < off; ++n) {
+            pos[n] = ctx_len[b] + dep[n];
+            /* chase parents up to the root, setting one bit per ancestor (and the self bit) */
+            for (int32_t a = n; a >= 0; a = par[a]) mk[(size_t)n * W + a / 32] |= (1u << (a % 32));
+        }
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Stage (c): verification attention, explicit definition.
+ * every tree query attends to the shared committed prefix and to its own
+ * candidate's in-block tokens ("cascade attention" is an exact re-association of this).
+ * For request b, node t, head h, kv head g = h / (Hq/Hkv) [G15]:
+ *   key set = { prefix j in [0,L_b) }  U  { tree a : bit a of mask row t }
+ *   s = (q . k) * sm_scale ;  m = max s ;  l = sum e^(s-m) ;  O = sum e^(s-m) v / l ;
+ *   LSE = m + ln l (natural log [G16]).
+ * which: 0 = full key set, 1 = prefix only, 2 = tree only.  Empty key set (prefix-only with L=0):
+ * O = 0, LSE = -inf.
+ * KV addressing: page_size == 0 -> contiguous rows kv_indptr[b] + j (kv_indptr NULL => 0);
+ * page_size > 0 -> page = kv_indices[kv_indptr[b] + j/page_size], row = page*page_size + j%page_size.
+ * ------------------------------------------------------------------------------------------ */
+static void attend_one(int which, const uint16_t* q, const uint16_t* k_cache, const uint16_t* v_cache,
+                       const int32_t* kv_indptr, const int32_t* kv_indices, int32_t page_size,
+                       const int32_t* ctx_len, const uint16_t* tree_k, const uint16_t* tree_v,
+                       const uint32_t* mask, int32_t T_cap, int32_t W, int32_t Hq, int32_t Hkv,
+                       int32_t d, double sm_scale, int32_t b, int32_t t, int32_t h, double* out,
+                       double* lse) {
+    int32_t g = h / (Hq / Hkv);
+    int32_t L = (which == 2) ? 0 : ctx_len[b];
+    int32_t nt = (which == 1) ? 0 : T_cap;
+    const uint16_t* qrow = q + (((size_t)b * T_cap + t) * Hq + h) * d;
+    const uint32_t* mrow = mask + ((size_t)b * T_cap + t) * W;
+    size_t cap = (size_t)L + (size_t)nt + 1;
+    double* s = (double*)malloc(sizeof(double) * cap);
+    const uint16_t** vptr = (const uint16_t**)malloc(sizeof(uint16_t*) * cap);
+    size_t n = 0;
+    for (int32_t j = 0; j < L; ++j) {
+        size_t row;
+        if (page_size > 0) {
+            int32_t page = kv_indices[(size_t)kv_indptr[b] + j / page_size];
+            row = (size_t)page * page_size + (size_t)(j % page_size);
+        } else {
+            row = (size_t)(kv_indptr ? kv_indptr[b] : 0) + (size_t)j;
+        }
+        const uint16_t* kr = k_cache + (row * Hkv + g) * d;
+        double acc = 0.0;
+        for (int32_t e = 0; e < d; ++e) acc += bf16_to_f64(qrow[e]) * bf16_to_f64(kr[e]);
+        s[n] = acc * sm_scale;
+        vptr[n] = v_cache + (row * Hkv + g) * d;
+        ++n;
+    }
+    for (int32_t a = 0; a < nt; ++a) {
+        if (!((mrow[a / 32] >> (a % 32)) & 1u)) continue;
+        const uint16_t* kr = tree_k + (((size_t)b * T_cap + a) * Hkv + g) * d;
+        double acc = 0.0;
+        for (int32_t e = 0; e < d; ++e) acc += bf16_to_f64(qrow[e]) * bf16_to_f64(kr[e]);
+        s[n] = acc * sm_scale;
+        vptr[n] = tree_v + (((size_t)b * T_cap + a) * Hkv + g) * d;
+        ++n;
+    }
+    for (int32_t e = 0; e < d; ++e) out[e] = 0.0;
+    if (n == 0) {
+        *lse = -INFINITY;
+    } else {
+        double m = s[0];
+        for (size_t i = 1; i < n; ++i) if (s[i] > m) m = s[i];
+        double l = 0.0;
+        for (size_t i = 0; i < n; ++i) l += exp(s[i] - m);
+        for (size_t i = 0; i < n; ++i) {
+            double p = exp(s[i] - m) / l;
+            for (int32_t e = 0; e < d; ++e) out[e] += p * bf16_to_f64(vptr[i][e]);
+        }
+        *lse = m + log(l);
+    }
+    free(s);
+    free(vptr);
+}
+
+/* Attention for a list of (b,t,h) triples (sel [n_sel,3]); out [n_sel,d], lse [n_sel]. */
+void d2sd_oracle_attention_rows(int32_t which, const uint16_t* q, const uint16_t* k_cache,
+                                const uint16_t* v_cache, const int32_t* kv_indptr,
+                                const int32_t* kv_indices, int32_t page_size, const int32_t* ctx_len,
+                                const uint16_t* tree_k, const uint16_t* tree_v, const uint32_t* mask,
+                                int32_t T_cap, int32_t W, int32_t Hq, int32_t Hkv, int32_t d,
+                                double sm_scale, const int32_t* sel, int64_t n_sel, double* out,
+                                double* lse) {
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t i = 0; i < n_sel; ++i) {
+        attend_one(which, q, k_cache, v_cache, kv_indptr, kv_indices, page_size, ctx_len, tree_k,
+                   tree_v, mask, T_cap, W, Hq, Hkv, d, sm_scale, sel[3 * i], sel[3 * i + 1],
+                   sel[3 * i + 2], out + (size_t)i * d, lse + i);
+    }
+}
+
+/* Attention for every (b, t < tree_len[b], h); out [B,T_cap,Hq,d], lse [B,T_cap,Hq].
+ * Rows t >= tree_len[b] are left untouched. */
+void d2sd_oracle_attention(int32_t which, const uint16_t* q, const uint16_t* k_cache,
+                           const uint16_t* v_cache, const int32_t* kv_indptr,
+                           const int32_t* kv_indices, int32_t page_size, const int32_t* ctx_len,
+                           const uint16_t* tree_k, const uint16_t* tree_v, const uint32_t* mask,
+                           const int32_t* tree_len, int32_t B, int32_t T_cap, int32_t W, int32_t Hq,
+                           int32_t Hkv, int32_t d, double sm_scale, double* out, double* lse) {
+    int64_t total = (int64_t)B * T_cap * Hq;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t i = 0; i < total; ++i) {
+        int32_t h = (int32_t)(i % Hq);
+        int32_t t = (int32_t)((i / Hq) % T_cap);
+        int32_t b = (int32_t)(i / ((int64_t)Hq * T_cap));
+        if (t >= tree_len[b]) continue;
+        attend_one(which, q, k_cache, v_cache, kv_indptr, kv_indices, page_size, ctx_len, tree_k,
+                   tree_v, mask, T_cap, W, Hq, Hkv, d, sm_scale, b, t, h, out + (size_t)i * d,
+                   lse + i);
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Stage (d): greedy acceptance.
+ * "accepting tokens up to (but not including) the first mismatch"; :124: "a
+ * longest-accepted-prefix search across branches ... the target's prediction at the rejection
+ * position becomes the next anchor".
+ * a[n] = first index of the maximum of logits[n,.] under IEEE comparison (-0 == +0) [G18].
+ * ok[0] = 1; ok[n] = ok[parent[n]] && tokens[n] == a[parent[n]]; best = deepest ok node, ties ->
+ * smallest node index [G17]; accept_len = depth[best] (accepted DRAFT tokens, anchor excluded
+ * [G19]); path = node ids root..best, -1 padded to gamma; bonus = a[best].
+ * logits bf16 bits, row n of request b at logits + (b*T_cap + n)*row_stride.
+ * ------------------------------------------------------------------------------------------ */
+void d2sd_oracle_argmax(const uint16_t* logits, int64_t row_stride, int32_t V, const int32_t* tree_len,
+                        int32_t B, int32_t T_cap, int32_t* argmax_out) {
+    int64_t total = (int64_t)B * T_cap;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t i = 0; i < total; ++i) {
+        int32_t b = (int32_t)(i / T_cap), n = (int32_t)(i % T_cap);
+        if (n >= tree_len[b]) { argmax_out[i] = -1; continue; }
+        const uint16_t* row = logits + (size_t)i * row_stride;
+        int32_t best = 0;
+        double bv = bf16_to_f64(row[0]);
+        for (int32_t v = 1; v < V; ++v) {
+            double x = bf16_to_f64(row[v]);
+            if (x > bv) { bv = x; best = v; }
+        }
+        argmax_out[i] = best;
+    }
+}
+
+void d2sd_oracle_accept_walk(const int32_t* argmax, const int32_t* tokens, const int32_t* parent,
+                             const int32_t* depth, const int32_t* tree_len, int32_t B, int32_t gamma,
+                             int32_t T_cap, int32_t* accept_len, int32_t* path, int32_t* bonus,
+                             int32_t* best_node) {
+    uint8_t* ok = (uint8_t*)malloc((size_t)T_cap);
+    for (int32_t b = 0; b < B; ++b) {
+        const int32_t* a = argmax + (size_t)b * T_cap;
+        const int32_t* tok = tokens + (size_t)b * T_cap;
+        const int32_t* par = parent + (size_t)b * T_cap;
+        const int32_t* dep = depth + (size_t)b * T_cap;
+        int32_t T = tree_len[b];
+        int32_t best = 0;
+        ok[0] = 1;
+        for (int32_t n = 1; n < T; ++n) {
+            ok[n] = (uint8_t)(ok[par[n]] && tok[n] == a[par[n]]); /* parent[n] < n always */
+            if (ok[n] && dep[n] > dep[best]) best = n;            /* strict: ties keep smaller n */
+        }
+        accept_len[b] = dep[best];
+        best_node[b] = best;
+        bonus[b] = a[best];
+        int32_t* pth = path + (size_t)b * gamma;
+        for (int32_t j = 0; j < gamma; ++j) pth[j] = -1;
+        for (int32_t n = best; n >= 0; n = par[n]) pth[dep[n]] = n;
+    }
+    free(ok);
+}
+
+/* Number of OpenMP threads the parallel loops above will use (reported by bench.py). */
+#ifdef _OPENMP
+#include <omp.h>
+int32_t d2sd_oracle_num_threads(void) { return (int32_t)omp_get_max_threads(); }
+#else
+int32_t d2sd_oracle_num_threads(void) { return 1; }
+#endif
