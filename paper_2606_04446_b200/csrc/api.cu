@@ -1,0 +1,216 @@
+// extern "C" entry points of libd2sd (declared and documented in include/d2sd.h): argument checks,
+// launch planning, kernel enqueue.  No allocation, no synchronisation, no host reads of device data.
+#include <cmath>
+#include <cstring>
+
+#include "common.cuh"
+
+namespace d2sd {
+
+static thread_local char g_err[512] = "";
+
+int32_t set_error(int32_t status, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof g_err, fmt, ap);
+    va_end(ap);
+    return status;
+}
+void clear_error() { g_err[0] = '\0'; }
+
+int sm_count() {
+    static int n = 0;
+    if (n == 0) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess ||
+            cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0)
+            n = 148;  // B200
+    }
+    return n;
+}
+
+static int32_t check_block(int32_t B, int32_t gamma, int32_t K) {
+    D2SD_CHECK_ARG(B >= 0, "B = %d must be >= 0", B);
+    D2SD_CHECK_ARG(gamma >= 2 && gamma <= 64, "gamma = %d outside [2,64]", gamma);
+    D2SD_CHECK_ARG(K >= 0 && K <= gamma - 1, "K = %d outside [0,gamma-1] (gamma = %d)", K, gamma);
+    return D2SD_OK;
+}
+
+// Split-KV plan.  chunk_keys is a multiple of 64 (the key-tile size of both prefix kernels).
+static int32_t make_plan(const d2sd_attn_params* p, AttnPlan* out) {
+    D2SD_CHECK_ARG(p != nullptr, "params is NULL");
+    D2SD_CHECK_ARG(p->B >= 0 && p->T_cap >= 1, "B = %d, T_cap = %d", p->B, p->T_cap);
+    D2SD_CHECK_ARG(p->Hq >= 1 && p->Hkv >= 1 && p->Hq % p->Hkv == 0, "Hq = %d not a multiple of Hkv = %d",
+                   p->Hq, p->Hkv);
+    D2SD_CHECK_ARG(p->max_ctx_len >= 0 && p->kv_rows >= 0, "max_ctx_len = %d, kv_rows = %lld",
+                   p->max_ctx_len, (long long)p->kv_rows);
+    D2SD_CHECK_ARG(p->num_splits >= 0 && p->impl >= 0 && p->impl <= 2, "num_splits = %d, impl = %d",
+                   p->num_splits, p->impl);
+    D2SD_CHECK_ARG(p->phases >= 0 && p->phases <= 7, "phases = %d outside [0,7]", p->phases);
+    D2SD_CHECK_SUPPORTED(p->d == 128, "head dim %d: only 128 is built", p->d);
+    D2SD_CHECK_SUPPORTED(p->page_size == 0 || p->page_size == 16, "page_size %d: only 0 (contiguous) or 16",
+                         p->page_size);
+    D2SD_CHECK_SUPPORTED(p->T_cap <= 1024, "T_cap = %d > 1024", p->T_cap);
+    D2SD_CHECK_SUPPORTED((int64_t)p->B * p->Hkv <= 65535, "B*Hkv = %lld > 65535", (long long)p->B * p->Hkv);
+    AttnPlan pl{};
+    pl.B = p->B; pl.T_cap = p->T_cap; pl.W = (p->T_cap + 31) / 32;
+    pl.Hq = p->Hq; pl.Hkv = p->Hkv; pl.G = p->Hq / p->Hkv; pl.d = p->d;
+    pl.sm_scale = p->sm_scale > 0.f ? p->sm_scale : 1.0f / sqrtf((float)p->d);
+    pl.page_size = p->page_size;
+    pl.max_ctx_len = p->max_ctx_len;
+    pl.kv_rows = p->kv_rows;
+    pl.use_tc = false;
+    if (p->impl != 1) {
+        pl.use_tc = attn_prefix_tc_supported(pl);
+        D2SD_CHECK_SUPPORTED(pl.use_tc || p->impl != 2, "impl = 2 (tcgen05) does not cover this shape");
+    }
+    const int rows = pl.T_cap * pl.G;
+    const int max_ctx = p->max_ctx_len > 0 ? p->max_ctx_len : 1;
+    int splits = p->num_splits;
+    if (splits == 0) {
+        // one wave of CTAs: the tcgen05 kernel is 1 CTA/SM with all (<= 3) M tiles of a kv head in
+        // one CTA; the mma.sync kernel runs ~3 CTAs/SM with 64-row M blocks.
+        const int64_t per_split = pl.use_tc ? (int64_t)pl.B * pl.Hkv * ceil_div(rows, 384)
+                                            : (int64_t)pl.B * pl.Hkv * ceil_div(rows, 64);
+        const int64_t target = pl.use_tc ? sm_count() : 3 * sm_count();
+        splits = (int)(target / (per_split > 0 ? per_split : 1));
+        if (splits < 1) splits = 1;
+        // never cut below 128 keys per chunk: the partial state would outweigh the KV it covers
+        const int max_splits = (max_ctx + 127) / 128;
+        if (splits > max_splits) splits = max_splits;
+        if (splits > 64) splits = 64;
+    }
+    int chunk = (ceil_div(max_ctx, splits) + 63) / 64 * 64;
+    pl.chunk_keys = chunk;
+    pl.num_splits = ceil_div(max_ctx, chunk);
+    pl.NS = pl.num_splits + 1;
+    const size_t rows_all = (size_t)pl.B * pl.NS * pl.T_cap * pl.Hq;
+    pl.off_o = 0;
+    pl.off_lse = align_up(rows_all * pl.d * sizeof(float), 256);
+    pl.bytes = pl.off_lse + align_up(rows_all * sizeof(float), 256);
+    *out = pl;
+    return D2SD_OK;
+}
+
+}  // namespace d2sd
+
+using namespace d2sd;
+
+extern "C" {
+
+const char* d2sd_last_error(void) { return g_err; }
+const char* d2sd_version(void) { return "d2sd 0.1 sm_100a"; }
+
+int32_t d2sd_select_prefixes(const float* conf, int32_t B, int32_t gamma, int32_t K, int32_t* prefix_len,
+                             double* r_out, void* stream) {
+    clear_error();
+    if (int32_t st = check_block(B, gamma, K)) return st;
+    D2SD_CHECK_ARG(B == 0 || conf != nullptr, "conf is NULL");
+    D2SD_CHECK_ARG(B == 0 || K == 0 || prefix_len != nullptr, "prefix_len is NULL");
+    return launch_select(conf, B, gamma, K, prefix_len, r_out, static_cast<cudaStream_t>(stream));
+}
+
+int32_t d2sd_build_tree(const int32_t* draft1, const int32_t* draft2, const int32_t* prefix_len,
+                        const int32_t* ctx_len, int32_t B, int32_t gamma, int32_t K, int32_t T_cap,
+                        int32_t* tokens, int32_t* parent, int32_t* depth, int32_t* pos_id,
+                        int32_t* branch_off, uint32_t* mask, int32_t* tree_len, void* stream) {
+    clear_error();
+    if (int32_t st = check_block(B, gamma, K)) return st;
+    const int need = gamma + K * (gamma - 1) - K * (K - 1) / 2;
+    D2SD_CHECK_ARG(T_cap >= need, "T_cap = %d < largest tree %d for gamma = %d, K = %d", T_cap, need, gamma, K);
+    D2SD_CHECK_SUPPORTED(T_cap <= 1024, "T_cap = %d > 1024", T_cap);
+    if (B == 0) return D2SD_OK;
+    D2SD_CHECK_ARG(draft1 && ctx_len && tokens && parent && depth && pos_id && branch_off && mask && tree_len,
+                   "a required buffer is NULL");
+    D2SD_CHECK_ARG(K == 0 || (draft2 && prefix_len), "draft2 / prefix_len is NULL with K = %d", K);
+    return launch_build_tree(draft1, draft2, prefix_len, ctx_len, B, gamma, K, T_cap, tokens, parent, depth,
+                             pos_id, branch_off, mask, tree_len, static_cast<cudaStream_t>(stream));
+}
+
+size_t d2sd_cascade_workspace_bytes(const d2sd_attn_params* p) {
+    clear_error();
+    AttnPlan pl;
+    if (make_plan(p, &pl) != D2SD_OK) return 0;
+    return pl.bytes;
+}
+
+int32_t d2sd_cascade_verify_attn(const d2sd_attn_params* p, const void* q, const void* k_cache,
+                                 const void* v_cache, const int32_t* kv_indptr, const int32_t* kv_indices,
+                                 const int32_t* ctx_len, const void* tree_k, const void* tree_v,
+                                 const uint32_t* mask, const int32_t* tree_len, void* out, float* lse,
+                                 float* dbg_state, void* workspace, size_t workspace_bytes, void* stream) {
+    clear_error();
+    AttnPlan pl;
+    if (int32_t st = make_plan(p, &pl)) return st;
+    if (pl.B == 0) return D2SD_OK;
+    D2SD_CHECK_ARG(q && ctx_len && tree_k && tree_v && mask && tree_len && out, "a required buffer is NULL");
+    D2SD_CHECK_ARG(p->max_ctx_len == 0 || (k_cache && v_cache), "k_cache / v_cache is NULL");
+    D2SD_CHECK_ARG(kv_indptr != nullptr || (pl.B == 1 && pl.page_size == 0),
+                   "kv_indptr may be NULL only for B == 1 contiguous KV");
+    D2SD_CHECK_ARG((pl.page_size > 0) == (kv_indices != nullptr),
+                   "kv_indices must be given exactly when page_size > 0");
+    const uintptr_t al = reinterpret_cast<uintptr_t>(q) | reinterpret_cast<uintptr_t>(k_cache) |
+                         reinterpret_cast<uintptr_t>(v_cache) | reinterpret_cast<uintptr_t>(tree_k) |
+                         reinterpret_cast<uintptr_t>(tree_v) | reinterpret_cast<uintptr_t>(out);
+    D2SD_CHECK_ARG((al & 15) == 0, "q/k_cache/v_cache/tree_k/tree_v/out must be 16-byte aligned");
+    if (workspace == nullptr || workspace_bytes < pl.bytes || (reinterpret_cast<uintptr_t>(workspace) & 255))
+        return set_error(D2SD_ERR_WORKSPACE, "workspace %p with %zu bytes; need %zu bytes, 256-byte aligned",
+                         workspace, workspace_bytes, pl.bytes);
+    AttnArgs a{};
+    a.q = static_cast<const __nv_bfloat16*>(q);
+    a.k_cache = static_cast<const __nv_bfloat16*>(k_cache);
+    a.v_cache = static_cast<const __nv_bfloat16*>(v_cache);
+    a.tree_k = static_cast<const __nv_bfloat16*>(tree_k);
+    a.tree_v = static_cast<const __nv_bfloat16*>(tree_v);
+    a.kv_indptr = kv_indptr; a.kv_indices = kv_indices; a.ctx_len = ctx_len; a.tree_len = tree_len;
+    a.mask = mask;
+    a.out = static_cast<__nv_bfloat16*>(out);
+    a.lse = lse; a.dbg_state = dbg_state;
+    a.part_o = reinterpret_cast<float*>(static_cast<char*>(workspace) + pl.off_o);
+    a.part_lse = reinterpret_cast<float*>(static_cast<char*>(workspace) + pl.off_lse);
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    const int phases = p->phases ? p->phases : 7;
+    const bool do_prefix = phases & 1, do_tree = phases & 2, do_merge = phases & 4;
+    if (pl.use_tc) {
+        if (do_prefix)
+            if (int32_t st = launch_attn_prefix_tc(pl, a, s)) return st;
+        if (do_tree)
+            if (int32_t st = launch_attn_mma(pl, a, /*prefix=*/false, /*tree=*/true, s)) return st;
+    } else if (do_prefix || do_tree) {
+        if (int32_t st = launch_attn_mma(pl, a, do_prefix, do_tree, s)) return st;
+    }
+    if (do_merge) return launch_attn_merge(pl, a, s);
+    return D2SD_OK;
+}
+
+size_t d2sd_accept_workspace_bytes(int32_t B, int32_t T_cap, int32_t V) {
+    if (B < 0 || T_cap < 1 || V < 1) return 0;
+    return align_up((size_t)B * T_cap * ceil_div(V, kArgmaxChunk) * 8, 256) + 256;
+}
+
+int32_t d2sd_accept(const void* logits, int64_t row_stride, int32_t V, const int32_t* tokens,
+                    const int32_t* parent, const int32_t* depth, const int32_t* tree_len, int32_t B,
+                    int32_t gamma, int32_t T_cap, int32_t* argmax_out, int32_t* accept_len, int32_t* path,
+                    int32_t* bonus, int32_t* best_node, void* workspace, size_t workspace_bytes,
+                    void* stream) {
+    clear_error();
+    D2SD_CHECK_ARG(B >= 0 && V >= 1 && row_stride >= V, "B = %d, V = %d, row_stride = %lld", B, V,
+                   (long long)row_stride);
+    D2SD_CHECK_ARG(gamma >= 2 && gamma <= 64, "gamma = %d outside [2,64]", gamma);
+    D2SD_CHECK_ARG(T_cap >= 1, "T_cap = %d", T_cap);
+    D2SD_CHECK_SUPPORTED(T_cap <= 1024, "T_cap = %d > 1024", T_cap);
+    D2SD_CHECK_SUPPORTED(ceil_div(V, kArgmaxChunk) <= 65535, "V = %d too large", V);
+    if (B == 0) return D2SD_OK;
+    D2SD_CHECK_ARG(logits && tokens && parent && depth && tree_len && argmax_out && accept_len && path &&
+                       bonus && best_node,
+                   "a required buffer is NULL");
+    if (workspace == nullptr || workspace_bytes < d2sd_accept_workspace_bytes(B, T_cap, V) ||
+        (reinterpret_cast<uintptr_t>(workspace) & 15))
+        return set_error(D2SD_ERR_WORKSPACE, "accept workspace %p with %zu bytes; need %zu, 16-byte aligned",
+                         workspace, workspace_bytes, d2sd_accept_workspace_bytes(B, T_cap, V));
+    return launch_accept(static_cast<const __nv_bfloat16*>(logits), row_stride, V, tokens, parent, depth,
+                         tree_len, B, gamma, T_cap, argmax_out, accept_len, path, bonus, best_node, workspace,
+                         static_cast<cudaStream_t>(stream));
+}
+
+}  // extern "C"

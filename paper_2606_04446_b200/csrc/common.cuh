@@ -1,0 +1,96 @@
+// Shared host/device helpers of libd2sd (CUDA side only; the CPU oracle shares nothing with this).
+#pragma once
+
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+
+#include <cstdarg>
+#include <cstdint>
+#include <cstdio>
+
+#include "d2sd.h"
+
+namespace d2sd {
+
+// Thread-local last-error text behind d2sd_last_error().
+int32_t set_error(int32_t status, const char* fmt, ...);
+void clear_error();
+
+#define D2SD_CHECK_ARG(cond, ...)                                         \
+    do {                                                                  \
+        if (!(cond)) return ::d2sd::set_error(D2SD_ERR_INVALID_ARG, __VA_ARGS__); \
+    } while (0)
+
+#define D2SD_CHECK_SUPPORTED(cond, ...)                                   \
+    do {                                                                  \
+        if (!(cond)) return ::d2sd::set_error(D2SD_ERR_UNSUPPORTED, __VA_ARGS__); \
+    } while (0)
+
+#define D2SD_CHECK_CUDA(expr)                                                                  \
+    do {                                                                                       \
+        cudaError_t _e = (expr);                                                               \
+        if (_e != cudaSuccess)                                                                 \
+            return ::d2sd::set_error(D2SD_ERR_CUDA, "%s failed: %s", #expr, cudaGetErrorString(_e)); \
+    } while (0)
+
+// Launch check that is legal during stream capture (no synchronisation).
+#define D2SD_CHECK_LAUNCH(name)                                                                \
+    do {                                                                                       \
+        cudaError_t _e = cudaPeekAtLastError();                                                \
+        if (_e != cudaSuccess) {                                                               \
+            (void)cudaGetLastError();                                                          \
+            return ::d2sd::set_error(D2SD_ERR_CUDA, "launch of %s failed: %s", name,           \
+                                     cudaGetErrorString(_e));                                  \
+        }                                                                                      \
+    } while (0)
+
+inline int ceil_div(int a, int b) { return (a + b - 1) / b; }
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+int sm_count();  // cached multiprocessor count of the current device
+
+// ---- stage launchers (defined in the per-stage .cu files) -------------------------------------
+int32_t launch_select(const float* conf, int B, int gamma, int K, int32_t* prefix_len, double* r_out,
+                      cudaStream_t s);
+int32_t launch_build_tree(const int32_t* draft1, const int32_t* draft2, const int32_t* prefix_len,
+                          const int32_t* ctx_len, int B, int gamma, int K, int T_cap, int32_t* tokens,
+                          int32_t* parent, int32_t* depth, int32_t* pos_id, int32_t* branch_off,
+                          uint32_t* mask, int32_t* tree_len, cudaStream_t s);
+
+constexpr int kArgmaxChunk = 8192;  // vocabulary elements scanned per CTA
+int32_t launch_accept(const __nv_bfloat16* logits, int64_t row_stride, int V, const int32_t* tokens,
+                      const int32_t* parent, const int32_t* depth, const int32_t* tree_len, int B,
+                      int gamma, int T_cap, int32_t* argmax_out, int32_t* accept_len, int32_t* path,
+                      int32_t* bonus, int32_t* best_node, void* workspace, cudaStream_t s);
+
+// Partial softmax states in the workspace: O fp32 [B][NS][T_cap][Hq][d], LSE fp32 [B][NS][T_cap][Hq];
+// slots 0..num_splits-1 are the prefix chunks, slot num_splits is the tree pass.
+struct AttnPlan {
+    int B, T_cap, W, Hq, Hkv, G, d;
+    float sm_scale;
+    int page_size;
+    int max_ctx_len;
+    int64_t kv_rows;
+    int num_splits;   // prefix chunks
+    int chunk_keys;   // keys per chunk (multiple of 64)
+    int NS;           // num_splits + 1
+    bool use_tc;      // tcgen05 prefix pass
+    size_t off_o, off_lse, bytes;
+};
+
+struct AttnArgs {
+    const __nv_bfloat16 *q, *k_cache, *v_cache, *tree_k, *tree_v;
+    const int32_t *kv_indptr, *kv_indices, *ctx_len, *tree_len;
+    const uint32_t* mask;
+    __nv_bfloat16* out;
+    float *lse, *dbg_state;
+    float *part_o, *part_lse;
+};
+
+int32_t launch_attn_mma(const AttnPlan& pl, const AttnArgs& a, bool do_prefix, bool do_tree,
+                        cudaStream_t s);
+int32_t launch_attn_merge(const AttnPlan& pl, const AttnArgs& a, cudaStream_t s);
+int32_t launch_attn_prefix_tc(const AttnPlan& pl, const AttnArgs& a, cudaStream_t s);
+bool attn_prefix_tc_supported(const AttnPlan& pl);
+
+}  // namespace d2sd

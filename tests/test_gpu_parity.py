@@ -1,0 +1,340 @@
+"""GPU parity: the CUDA path (through the C ABI binding) against the CPU oracle, same seeded inputs.
+
+Bit-exact for selection, tree indices, masks, argmax and acceptance; attention within
+2e-2 abs / 1e-2 rel per element, LSE within 1e-3 (BASELINE.json) plus the stricter row / state
+gates of DESIGN.md ("Tolerances"), because the stated gate is nearly vacuous at long context.
+"""
+import numpy as np
+import pytest
+import torch
+
+import d2sd_synth as synth
+from helpers import (STATE_REL_L2, bf16_cuda, check_rows, gpu_attention, i32_cuda, mask_cuda, oracle_tree,
+                     valid_rows)
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def d2sd():
+    import paper_2606_04446_b200 as m
+    m.lib()  # fails loudly if libd2sd.so is missing
+    assert torch.cuda.is_available()
+    return m
+
+
+# ------------------------------------------------------------------------------------------ (a)
+
+@pytest.mark.parametrize("gamma,K", [(2, 0), (2, 1), (4, 2), (6, 4), (16, 2), (16, 4), (16, 15), (32, 8), (64, 4), (64, 63)])
+def test_select_bit_exact(d2sd, oracle, gamma, K):
+    rng = np.random.default_rng(1000 + gamma * 64 + K)
+    conf = rng.random((257, gamma), dtype=np.float32)
+    conf[0, 1:] = 1.0                      # every r(i) == 0: pure tie-break
+    conf[1, 1:] = 0.5
+    if gamma > 2:
+        conf[2, 1] = 0.0                   # r(0) = 1, rest exactly 0
+        conf[3, 1:] = rng.choice([0.0, 0.25, 0.5, 1.0], gamma - 1)
+        conf[4, 1:] = 1e-30                # underflow-prone in fp32, fine in fp64
+    pl_ref, r_ref = oracle.select_prefixes(conf, K)
+    r = torch.empty((257, gamma - 1), dtype=torch.float64, device="cuda")
+    pl = d2sd.select_prefixes(torch.from_numpy(conf).cuda(), K, r_out=r)
+    torch.cuda.synchronize()
+    assert np.array_equal(r.cpu().numpy().view(np.uint64), r_ref.view(np.uint64)), "r(i) not bit-identical"
+    assert np.array_equal(pl.cpu().numpy(), pl_ref)
+
+
+# ------------------------------------------------------------------------------------------ (b)
+
+@pytest.mark.parametrize("gamma,K", [(2, 0), (2, 1), (4, 2), (6, 4), (16, 0), (16, 2), (16, 4), (16, 15), (32, 8), (64, 3)])
+def test_build_tree_bit_exact(d2sd, oracle, gamma, K):
+    rng = np.random.default_rng(2000 + gamma * 64 + K)
+    B = 9
+    conf = rng.random((B, gamma), dtype=np.float32)
+    pl, _ = oracle.select_prefixes(conf, K)
+    d1 = rng.integers(0, 151936, (B, gamma), dtype=np.int32)
+    d2 = rng.integers(0, 151936, (B, K, gamma), dtype=np.int32)
+    ctx = rng.integers(0, 40000, (B,), dtype=np.int32)
+    for T_cap in (synth.t_cap(gamma, K), synth.t_cap(gamma, K) + 37):
+        ref = oracle.build_tree(d1, d2, pl, ctx, T_cap)
+        got = d2sd.build_tree(i32_cuda(d1), i32_cuda(d2), i32_cuda(pl), i32_cuda(ctx), T_cap)
+        torch.cuda.synchronize()
+        for name in ("tokens", "parent", "depth", "pos_id", "branch_off", "tree_len"):
+            assert np.array_equal(got[name].cpu().numpy(), ref[name]), name
+        assert np.array_equal(got["mask"].cpu().numpy().view(np.uint32), ref["mask"]), "mask"
+
+
+def test_select_then_build_chain(d2sd, oracle):
+    """(a) feeding (b) on the device, no host round trip, all five config shapes."""
+    for n, cfg in synth.CONFIGS.items():
+        st = synth.make_step_inputs(cfg)
+        pl_ref, _, tree_ref = oracle_tree(oracle, cfg, st)
+        pl = d2sd.select_prefixes(torch.from_numpy(st["conf"]).cuda(), cfg.K)
+        got = d2sd.build_tree(i32_cuda(st["draft1"]), i32_cuda(st["draft2"]), pl, i32_cuda(st["ctx_len"]), cfg.T_cap)
+        torch.cuda.synchronize()
+        assert np.array_equal(pl.cpu().numpy(), pl_ref)
+        for name in ("tokens", "parent", "depth", "pos_id", "branch_off", "tree_len"):
+            assert np.array_equal(got[name].cpu().numpy(), tree_ref[name]), (n, name)
+        assert np.array_equal(got["mask"].cpu().numpy().view(np.uint32), tree_ref["mask"])
+
+
+# ------------------------------------------------------------------------------------------ (d)
+
+def _accept_case(d2sd, oracle, cfg, logits_bits, tree, gamma, row_stride=None):
+    B, T_cap, V = logits_bits.shape
+    ref = oracle.accept(logits_bits, tree["tokens"], tree["parent"], tree["depth"], tree["tree_len"], gamma)
+    lg = bf16_cuda(logits_bits)
+    if row_stride is not None:  # exercise a padded row stride (and a misaligned row start)
+        big = torch.zeros((B, T_cap, row_stride), dtype=torch.bfloat16, device="cuda")
+        big[:, :, :V] = lg
+        lg = big[:, :, :V]
+    got = d2sd.accept(lg, i32_cuda(tree["tokens"]), i32_cuda(tree["parent"]), i32_cuda(tree["depth"]),
+                      i32_cuda(tree["tree_len"]), gamma)
+    torch.cuda.synchronize()
+    for name in ("argmax", "accept_len", "bonus", "best_node", "path"):
+        assert np.array_equal(got[name].cpu().numpy(), ref[name]), name
+    return ref
+
+
+@pytest.mark.parametrize("cfg_no", [1, 2, 4])
+def test_accept_bit_exact_configs(d2sd, oracle, cfg_no):
+    cfg = synth.CONFIGS[cfg_no]
+    st = synth.make_step_inputs(cfg)
+    _, _, tree = oracle_tree(oracle, cfg, st)
+    for force in (None, 0.0, 1.0):
+        logits = synth.make_logits(cfg)
+        synth.plant_acceptance(cfg, logits, st["conf"], tree["tokens"], tree["parent"], tree["depth"],
+                               tree["tree_len"], force=force)
+        ref = _accept_case(d2sd, oracle, cfg, logits, tree, cfg.gamma)
+        if force == 0.0:
+            assert ref["accept_len"][0] >= 1
+        if force == 1.0:
+            assert ref["accept_len"][0] == 0
+
+
+def test_accept_ties_strides_and_small_vocab(d2sd, oracle):
+    rng = np.random.default_rng(77)
+    for V, stride in ((1, None), (7, None), (1024, None), (8191, 8200), (8193, 8195), (20001, 20003), (151936, None)):
+        cfg = synth.custom(50, B=3, gamma=8, K=3, V=V)
+        st = synth.make_step_inputs(cfg)
+        _, _, tree = oracle_tree(oracle, cfg, st)
+        logits = synth.make_logits(cfg)
+        T = cfg.T_cap
+        # planted ties: duplicate the row maximum at random later/earlier places; signed zeros; -inf rows
+        f = synth.bf16_bits_to_f32(logits)
+        for b in range(cfg.B):
+            for n in range(T):
+                if V > 4 and rng.random() < 0.5:
+                    mx = logits[b, n, np.argmax(f[b, n])]
+                    logits[b, n, rng.integers(0, V, 3)] = mx
+            logits[b, 1, :] = 0x8000
+            logits[b, 1, V // 2] = 0x0000
+            logits[b, 2, :] = 0xFF80  # -inf everywhere -> index 0
+        synth.plant_acceptance(cfg, logits, st["conf"], tree["tokens"], tree["parent"], tree["depth"],
+                               tree["tree_len"])
+        _accept_case(d2sd, oracle, cfg, logits, tree, cfg.gamma, row_stride=stride)
+
+
+def test_accept_duplicate_siblings_prefers_trunk(d2sd, oracle):
+    """G17: a branch head equal to its trunk sibling -> two equally long accepted paths."""
+    cfg = synth.custom(51, gamma=8, K=3, V=64)
+    st = synth.make_step_inputs(cfg)
+    pl, _ = oracle.select_prefixes(st["conf"], cfg.K)
+    for k in range(cfg.K):
+        st["draft2"][0, k, :] = st["draft1"][0, :]  # every branch re-drafts exactly the trunk tokens
+    tree = oracle.build_tree(st["draft1"], st["draft2"], pl, st["ctx_len"], cfg.T_cap)
+    logits = synth.make_logits(cfg)
+    synth.plant_acceptance(cfg, logits, np.ones_like(st["conf"]), tree["tokens"], tree["parent"], tree["depth"],
+                           tree["tree_len"], force=0.0)
+    ref = _accept_case(d2sd, oracle, cfg, logits, tree, cfg.gamma)
+    assert ref["best_node"][0] == cfg.gamma - 1 and ref["accept_len"][0] == cfg.gamma - 1
+
+
+# ------------------------------------------------------------------------------------------ (c)
+
+def _attn_full_case(d2sd, oracle, cfg, q_scale=1.0, layer=0, pool_nan=False, **kw):
+    st = synth.make_step_inputs(cfg)
+    _, _, tree = oracle_tree(oracle, cfg, st)
+    ti = synth.make_tree_inputs(cfg, layer, q_scale=q_scale)
+    kv = synth.make_kv_cache(cfg, st["ctx_len"], layer, pool_fill_nan=pool_nan)
+    o, lse, dbg = gpu_attention(d2sd, cfg, st, tree, ti, kv, dbg=True, **kw)
+    args = (ti["q"], kv["k_cache"], kv["v_cache"], kv["kv_indptr"], kv["kv_indices"], kv["page_size"],
+            st["ctx_len"], ti["tree_k"], ti["tree_v"], tree["mask"], tree["tree_len"])
+    ro, rl = oracle.attention(*args, which="full")
+    v = valid_rows(tree["tree_len"], cfg.T_cap)
+    check_rows(o[v], lse[v], ro[v], rl[v], f"cfg{cfg.number} full")
+    assert np.isnan(o[~v]).all() and np.isnan(lse[~v]).all(), "padding rows must stay untouched"
+    for idx, which in ((0, "prefix"), (1, "tree")):
+        so, sl = oracle.attention(*args, which=which)
+        check_rows(dbg[idx][v][..., :-1], dbg[idx][v][..., -1], so[v], sl[v], f"cfg{cfg.number} {which}-only",
+                   row_gate=STATE_REL_L2, elementwise=False)
+    return o, lse
+
+
+def test_attn_config1_full(d2sd, oracle):
+    _attn_full_case(d2sd, oracle, synth.CONFIGS[1])
+
+
+def test_attn_config1_peaked(d2sd, oracle):
+    """Q scaled x4: softmax concentrates, |O| is O(1) and the absolute gate bites."""
+    _attn_full_case(d2sd, oracle, synth.CONFIGS[1], q_scale=4.0)
+
+
+@pytest.mark.parametrize("L", [0, 1, 15, 16, 17, 63, 64, 65, 255])
+def test_attn_short_context_tree_dominates(d2sd, oracle, L):
+    cfg = synth.custom(60 + L % 7, gamma=16, K=4, ctx=(L, L))
+    _attn_full_case(d2sd, oracle, cfg)
+
+
+@pytest.mark.parametrize("splits", [1, 2, 3, 5, 8])
+def test_attn_split_sweep(d2sd, oracle, splits):
+    cfg = synth.custom(70, gamma=16, K=4, ctx=(1000, 1000))
+    _attn_full_case(d2sd, oracle, cfg, num_splits=splits)
+
+
+@pytest.mark.parametrize("gamma,K,Hq,Hkv", [(16, 0, 32, 8), (4, 2, 8, 8), (6, 4, 16, 2), (32, 8, 32, 8), (16, 4, 24, 8)])
+def test_attn_shapes(d2sd, oracle, gamma, K, Hq, Hkv):
+    cfg = synth.custom(80 + gamma + K, gamma=gamma, K=K, Hq=Hq, Hkv=Hkv, ctx=(333, 333))
+    _attn_full_case(d2sd, oracle, cfg)
+
+
+def test_attn_batched_contiguous_ragged(d2sd, oracle):
+    cfg = synth.custom(90, B=5, gamma=16, K=4, ctx=(0, 700))
+    _attn_full_case(d2sd, oracle, cfg)
+
+
+def test_attn_paged_ragged_reduced_config5(d2sd, oracle):
+    """Config 5 at reduced size: paged KV (page 16, random page table, partial tail pages), ragged
+    contexts; slots no request owns are NaN and must never reach an output."""
+    cfg = synth.custom(91, B=6, gamma=16, K=4, ctx=(1, 900), paged=True)
+    _attn_full_case(d2sd, oracle, cfg, pool_nan=True)
+
+
+def test_attn_config2_one_layer_full(d2sd, oracle):
+    """Config 2 shape (L=4096, T_cap=70), one of its 36 layers, every output element."""
+    cfg = synth.CONFIGS[2]
+    _attn_full_case(d2sd, oracle, cfg, layer=3)
+
+
+def _attn_sampled_case(d2sd, oracle, cfg, n_samples, layer=0):
+    st = synth.make_step_inputs(cfg)
+    _, _, tree = oracle_tree(oracle, cfg, st)
+    ti = synth.make_tree_inputs(cfg, layer)
+    kv = synth.make_kv_cache(cfg, st["ctx_len"], layer)
+    o, lse, dbg = gpu_attention(d2sd, cfg, st, tree, ti, kv, dbg=True)
+    sel = synth.sample_rows(cfg, tree["tree_len"], n_samples)
+    args = (ti["q"], kv["k_cache"], kv["v_cache"], kv["kv_indptr"], kv["kv_indices"], kv["page_size"],
+            st["ctx_len"], ti["tree_k"], ti["tree_v"], tree["mask"], sel)
+    ro, rl = oracle.attention_rows(*args, which="full")
+    b, t, h = sel[:, 0], sel[:, 1], sel[:, 2]
+    check_rows(o[b, t, h], lse[b, t, h], ro, rl, f"cfg{cfg.number} sampled full")
+    for idx, which in ((0, "prefix"), (1, "tree")):
+        so, sl = oracle.attention_rows(*args, which=which)
+        check_rows(dbg[idx][b, t, h][..., :-1], dbg[idx][b, t, h][..., -1], so, sl,
+                   f"cfg{cfg.number} sampled {which}-only", row_gate=STATE_REL_L2, elementwise=False)
+    v = valid_rows(tree["tree_len"], cfg.T_cap)
+    assert np.isfinite(o[v]).all() and np.isfinite(lse[v]).all()
+    assert np.isnan(o[~v]).all()
+
+
+def test_attn_config3_sampled(d2sd, oracle):
+    _attn_sampled_case(d2sd, oracle, synth.CONFIGS[3], 96)
+
+
+def test_attn_config4_sampled(d2sd, oracle):
+    _attn_sampled_case(d2sd, oracle, synth.CONFIGS[4], 192)
+
+
+def test_attn_config5_sampled(d2sd, oracle):
+    _attn_sampled_case(d2sd, oracle, synth.CONFIGS[5], 128)
+
+
+# ------------------------------------------------------------------------------------------ whole path
+
+def test_whole_path_config1(d2sd, oracle):
+    """select -> build -> attention -> accept, every stage fed by the previous one on the device."""
+    cfg = synth.CONFIGS[1]
+    st = synth.make_step_inputs(cfg)
+    pl_ref, _, tree_ref = oracle_tree(oracle, cfg, st)
+    ti = synth.make_tree_inputs(cfg)
+    kv = synth.make_kv_cache(cfg, st["ctx_len"])
+    logits = synth.make_logits(cfg)
+    synth.plant_acceptance(cfg, logits, st["conf"], tree_ref["tokens"], tree_ref["parent"], tree_ref["depth"],
+                           tree_ref["tree_len"])
+    pl = d2sd.select_prefixes(torch.from_numpy(st["conf"]).cuda(), cfg.K)
+    tree = d2sd.build_tree(i32_cuda(st["draft1"]), i32_cuda(st["draft2"]), pl, i32_cuda(st["ctx_len"]), cfg.T_cap)
+    out, lse = d2sd.cascade_verify_attn(
+        bf16_cuda(ti["q"]), bf16_cuda(kv["k_cache"]), bf16_cuda(kv["v_cache"]), None, None, i32_cuda(st["ctx_len"]),
+        bf16_cuda(ti["tree_k"]), bf16_cuda(ti["tree_v"]), tree["mask"], tree["tree_len"], int(st["ctx_len"].max()))
+    acc = d2sd.accept(bf16_cuda(logits), tree["tokens"], tree["parent"], tree["depth"], tree["tree_len"], cfg.gamma)
+    torch.cuda.synchronize()
+    ro, rl = oracle.attention(ti["q"], kv["k_cache"], kv["v_cache"], kv["kv_indptr"], None, 0, st["ctx_len"],
+                              ti["tree_k"], ti["tree_v"], tree_ref["mask"], tree_ref["tree_len"])
+    T = int(tree_ref["tree_len"][0])
+    check_rows(out.float().cpu().numpy()[0, :T], lse.cpu().numpy()[0, :T], ro[0, :T], rl[0, :T], "whole path")
+    ref = oracle.accept(logits, tree_ref["tokens"], tree_ref["parent"], tree_ref["depth"], tree_ref["tree_len"], cfg.gamma)
+    for name in ("argmax", "accept_len", "bonus", "best_node", "path"):
+        assert np.array_equal(acc[name].cpu().numpy(), ref[name]), name
+
+
+def test_graph_capture_whole_path(d2sd, oracle):
+    """The four calls are CUDA-graph capturable (pre-warmed CUDA graphs)."""
+    cfg = synth.CONFIGS[1]
+    st = synth.make_step_inputs(cfg)
+    _, _, tree_ref = oracle_tree(oracle, cfg, st)
+    ti = synth.make_tree_inputs(cfg)
+    kv = synth.make_kv_cache(cfg, st["ctx_len"])
+    logits = synth.make_logits(cfg)
+    synth.plant_acceptance(cfg, logits, st["conf"], tree_ref["tokens"], tree_ref["parent"], tree_ref["depth"],
+                           tree_ref["tree_len"])
+    conf, d1, d2c, ctx = torch.from_numpy(st["conf"]).cuda(), i32_cuda(st["draft1"]), i32_cuda(st["draft2"]), i32_cuda(st["ctx_len"])
+    q, kc, vc, tk, tv, lg = (bf16_cuda(x) for x in (ti["q"], kv["k_cache"], kv["v_cache"], ti["tree_k"], ti["tree_v"], logits))
+    ws = torch.empty(d2sd.cascade_workspace_bytes(cfg.B, cfg.T_cap, cfg.Hq, cfg.Hkv, cfg.d, 256), dtype=torch.uint8, device="cuda")
+    ws2 = torch.empty(d2sd.accept_workspace_bytes(cfg.B, cfg.T_cap, cfg.V), dtype=torch.uint8, device="cuda")
+    res = {}
+
+    def step():
+        pl = d2sd.select_prefixes(conf, cfg.K, prefix_len=res.get("pl"))
+        tree = d2sd.build_tree(d1, d2c, pl, ctx, cfg.T_cap, out=res.get("tree"))
+        out, lse = d2sd.cascade_verify_attn(q, kc, vc, None, None, ctx, tk, tv, tree["mask"], tree["tree_len"], 256,
+                                            out=res.get("out"), lse=res.get("lse"), workspace=ws)
+        acc = d2sd.accept(lg, tree["tokens"], tree["parent"], tree["depth"], tree["tree_len"], cfg.gamma,
+                          out=res.get("acc"), workspace=ws2)
+        res.update(pl=pl, tree=tree, out=out, lse=lse, acc=acc)
+
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        step()
+        torch.cuda.synchronize()
+        eager = {k: v.clone() for k, v in res["acc"].items()}
+        eager_out = res["out"].clone()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            step()
+        res["out"].zero_()
+        for v in res["acc"].values():
+            v.fill_(-5)
+        g.replay()
+        torch.cuda.synchronize()
+    T = int(tree_ref["tree_len"][0])
+    assert torch.equal(res["out"][0, :T], eager_out[0, :T])
+    for k in eager:
+        assert torch.equal(res["acc"][k], eager[k]), k
+
+
+# ------------------------------------------------------------------------------------------ errors
+
+def test_argument_errors(d2sd):
+    conf = torch.rand((2, 16), device="cuda")
+    with pytest.raises(d2sd.D2sdError):
+        d2sd.select_prefixes(conf, 16)          # K > gamma-1
+    with pytest.raises(d2sd.D2sdError):
+        d2sd.select_prefixes(torch.rand((2, 65), device="cuda"), 4)  # gamma > 64
+    with pytest.raises(d2sd.D2sdError):
+        d2sd.cascade_workspace_bytes(1, 70, 32, 8, 64, 4096)        # d != 128
+    with pytest.raises(d2sd.D2sdError):
+        d2sd.cascade_workspace_bytes(1, 70, 32, 7, 128, 4096)       # Hq % Hkv
+    z = torch.zeros((1, 16), dtype=torch.int32, device="cuda")
+    with pytest.raises(d2sd.D2sdError):                              # T_cap too small
+        d2sd.build_tree(z, torch.zeros((1, 4, 16), dtype=torch.int32, device="cuda"),
+                        torch.zeros((1, 4), dtype=torch.int32, device="cuda"),
+                        torch.zeros((1,), dtype=torch.int32, device="cuda"), T_cap=20)
