@@ -151,11 +151,27 @@ def test_accept_duplicate_siblings_prefers_trunk(d2sd, oracle):
 
 # ------------------------------------------------------------------------------------------ (c)
 
-def _attn_full_case(d2sd, oracle, cfg, q_scale=1.0, layer=0, pool_nan=False, **kw):
+IMPLS = [pytest.param(1, id="mma.sync"), pytest.param(0, id="auto-tcgen05")]
+
+
+def _ramp_keys(kv, ctx_len, lo=0.25, hi=4.0):
+    """Scale key j of every request by lo + (hi-lo)*j/L: the running maximum keeps rising along the
+    context, which forces the online-softmax rescale path (harness-side input shaping only)."""
+    k = synth.bf16_bits_to_f32(kv["k_cache"])
+    assert kv["page_size"] == 0
+    for b, L in enumerate(ctx_len):
+        s = int(kv["kv_indptr"][b])
+        k[s:s + L] *= (lo + (hi - lo) * np.arange(L, dtype=np.float32) / max(int(L), 1))[:, None, None]
+    kv["k_cache"] = synth.f32_to_bf16_bits(k)
+
+
+def _attn_full_case(d2sd, oracle, cfg, q_scale=1.0, layer=0, pool_nan=False, ramp=False, **kw):
     st = synth.make_step_inputs(cfg)
     _, _, tree = oracle_tree(oracle, cfg, st)
     ti = synth.make_tree_inputs(cfg, layer, q_scale=q_scale)
     kv = synth.make_kv_cache(cfg, st["ctx_len"], layer, pool_fill_nan=pool_nan)
+    if ramp:
+        _ramp_keys(kv, st["ctx_len"])
     o, lse, dbg = gpu_attention(d2sd, cfg, st, tree, ti, kv, dbg=True, **kw)
     args = (ti["q"], kv["k_cache"], kv["v_cache"], kv["kv_indptr"], kv["kv_indices"], kv["page_size"],
             st["ctx_len"], ti["tree_k"], ti["tree_v"], tree["mask"], tree["tree_len"])
@@ -170,36 +186,59 @@ def _attn_full_case(d2sd, oracle, cfg, q_scale=1.0, layer=0, pool_nan=False, **k
     return o, lse
 
 
-def test_attn_config1_full(d2sd, oracle):
-    _attn_full_case(d2sd, oracle, synth.CONFIGS[1])
+@pytest.mark.parametrize("impl", IMPLS)
+def test_attn_config1_full(d2sd, oracle, impl):
+    _attn_full_case(d2sd, oracle, synth.CONFIGS[1], impl=impl)
 
 
-def test_attn_config1_peaked(d2sd, oracle):
+@pytest.mark.parametrize("impl", IMPLS)
+def test_attn_config1_peaked(d2sd, oracle, impl):
     """Q scaled x4: softmax concentrates, |O| is O(1) and the absolute gate bites."""
-    _attn_full_case(d2sd, oracle, synth.CONFIGS[1], q_scale=4.0)
+    _attn_full_case(d2sd, oracle, synth.CONFIGS[1], q_scale=4.0, impl=impl)
 
 
+@pytest.mark.parametrize("impl", IMPLS)
+@pytest.mark.parametrize("splits", [1, 3])
+def test_attn_rising_scores_force_rescale(d2sd, oracle, impl, splits):
+    """Keys grow along the context so the row maximum rises tile after tile: exercises the lazy
+    online-softmax rescale of O (threshold 2^8) and its interplay with the split merge."""
+    cfg = synth.custom(73, gamma=16, K=4, ctx=(1500, 1500))
+    _attn_full_case(d2sd, oracle, cfg, q_scale=2.0, ramp=True, impl=impl, num_splits=splits)
+
+
+@pytest.mark.parametrize("impl", IMPLS)
 @pytest.mark.parametrize("L", [0, 1, 15, 16, 17, 63, 64, 65, 255])
-def test_attn_short_context_tree_dominates(d2sd, oracle, L):
+def test_attn_short_context_tree_dominates(d2sd, oracle, L, impl):
     cfg = synth.custom(60 + L % 7, gamma=16, K=4, ctx=(L, L))
-    _attn_full_case(d2sd, oracle, cfg)
+    _attn_full_case(d2sd, oracle, cfg, impl=impl)
 
 
+@pytest.mark.parametrize("impl", IMPLS)
 @pytest.mark.parametrize("splits", [1, 2, 3, 5, 8])
-def test_attn_split_sweep(d2sd, oracle, splits):
+def test_attn_split_sweep(d2sd, oracle, splits, impl):
     cfg = synth.custom(70, gamma=16, K=4, ctx=(1000, 1000))
-    _attn_full_case(d2sd, oracle, cfg, num_splits=splits)
+    _attn_full_case(d2sd, oracle, cfg, num_splits=splits, impl=impl)
 
 
+@pytest.mark.parametrize("impl", IMPLS)
 @pytest.mark.parametrize("gamma,K,Hq,Hkv", [(16, 0, 32, 8), (4, 2, 8, 8), (6, 4, 16, 2), (32, 8, 32, 8), (16, 4, 24, 8)])
-def test_attn_shapes(d2sd, oracle, gamma, K, Hq, Hkv):
+def test_attn_shapes(d2sd, oracle, gamma, K, Hq, Hkv, impl):
+    """G = 4, 1, 8, 4 and 3 (G = 3 does not divide a 128-row tile: auto falls back to mma.sync)."""
     cfg = synth.custom(80 + gamma + K, gamma=gamma, K=K, Hq=Hq, Hkv=Hkv, ctx=(333, 333))
-    _attn_full_case(d2sd, oracle, cfg)
+    _attn_full_case(d2sd, oracle, cfg, impl=impl)
 
 
-def test_attn_batched_contiguous_ragged(d2sd, oracle):
+@pytest.mark.parametrize("impl", IMPLS)
+def test_attn_batched_contiguous_ragged(d2sd, oracle, impl):
     cfg = synth.custom(90, B=5, gamma=16, K=4, ctx=(0, 700))
-    _attn_full_case(d2sd, oracle, cfg)
+    _attn_full_case(d2sd, oracle, cfg, impl=impl)
+
+
+def test_attn_tcgen05_is_the_default_for_contiguous_kv(d2sd):
+    """impl = 2 (force tcgen05) is accepted exactly where auto picks it; paged KV is not covered yet."""
+    assert d2sd.cascade_workspace_bytes(1, 70, 32, 8, 128, 4096, kv_rows=4096, impl=2) > 0
+    with pytest.raises(d2sd.D2sdError):
+        d2sd.cascade_workspace_bytes(1, 70, 32, 8, 128, 4096, page_size=16, kv_rows=8192, impl=2)
 
 
 def test_attn_paged_ragged_reduced_config5(d2sd, oracle):
@@ -209,10 +248,11 @@ def test_attn_paged_ragged_reduced_config5(d2sd, oracle):
     _attn_full_case(d2sd, oracle, cfg, pool_nan=True)
 
 
-def test_attn_config2_one_layer_full(d2sd, oracle):
+@pytest.mark.parametrize("impl", IMPLS)
+def test_attn_config2_one_layer_full(d2sd, oracle, impl):
     """Config 2 shape (L=4096, T_cap=70), one of its 36 layers, every output element."""
     cfg = synth.CONFIGS[2]
-    _attn_full_case(d2sd, oracle, cfg, layer=3)
+    _attn_full_case(d2sd, oracle, cfg, layer=3, impl=impl)
 
 
 def _attn_sampled_case(d2sd, oracle, cfg, n_samples, layer=0):
