@@ -67,27 +67,50 @@ static int32_t make_plan(const d2sd_attn_params* p, AttnPlan* out) {
     const int rows = pl.T_cap * pl.G;
     const int max_ctx = p->max_ctx_len > 0 ? p->max_ctx_len : 1;
     int splits = p->num_splits;
-    if (splits == 0) {
-        // one wave of CTAs: the tcgen05 kernel is 1 CTA/SM with all (<= 3) M tiles of a kv head in
-        // one CTA; the mma.sync kernel runs ~3 CTAs/SM with 64-row M blocks.
-        const int64_t per_split = pl.use_tc ? (int64_t)pl.B * pl.Hkv * ceil_div(rows, 384)
-                                            : (int64_t)pl.B * pl.Hkv * ceil_div(rows, 64);
-        const int64_t target = pl.use_tc ? sm_count() : 3 * sm_count();
-        splits = (int)(target / (per_split > 0 ? per_split : 1));
-        if (splits < 1) splits = 1;
-        // never cut below 128 keys per chunk: the partial state would outweigh the KV it covers
-        const int max_splits = (max_ctx + 127) / 128;
-        if (splits > max_splits) splits = max_splits;
-        if (splits > 64) splits = 64;
+    if (pl.use_tc) {
+        // One wave of CTA pairs (1 CTA/SM): a work item (request, kv head, group of <= 3 query tiles,
+        // chunk) is served by two CTAs.  Chunks are multiples of 16 keys (the MMA N granularity).
+        pl.n_mgroups = ceil_div(rows, 384);
+        pl.rows_pad = pl.n_mgroups * 384;
+        if (splits == 0) {
+            const int64_t per_split = (int64_t)pl.B * pl.Hkv * pl.n_mgroups;
+            splits = (int)((sm_count() / 2) / (per_split > 0 ? per_split : 1));
+            if (splits < 1) splits = 1;
+            const int max_splits = (max_ctx + 127) / 128;  // never below one 128-key tile per chunk
+            if (splits > max_splits) splits = max_splits;
+            if (splits > 64) splits = 64;
+        }
+        D2SD_CHECK_SUPPORTED(splits <= 16384, "num_splits = %d too large", splits);
+        pl.chunk_keys = (ceil_div(max_ctx, splits) + 15) / 16 * 16;
+        pl.num_splits = ceil_div(max_ctx, pl.chunk_keys);
+        pl.NSLOT = 2 * pl.num_splits;
+        pl.NS = 1;  // the tree state, row layout
+        const size_t slot_rows = (size_t)pl.B * pl.NSLOT * pl.Hkv * pl.rows_pad;
+        const size_t tree_rows = (size_t)pl.B * pl.T_cap * pl.Hq;
+        pl.off_o = 0;
+        pl.off_lse = align_up(slot_rows * pl.d * sizeof(float), 256);
+        pl.off_tree_o = pl.off_lse + align_up(slot_rows * sizeof(float), 256);
+        pl.off_tree_lse = pl.off_tree_o + align_up(tree_rows * pl.d * sizeof(float), 256);
+        pl.bytes = pl.off_tree_lse + align_up(tree_rows * sizeof(float), 256);
+    } else {
+        if (splits == 0) {
+            // ~3 CTAs/SM of 64-row M blocks
+            const int64_t per_split = (int64_t)pl.B * pl.Hkv * ceil_div(rows, 64);
+            splits = (int)(3 * sm_count() / (per_split > 0 ? per_split : 1));
+            if (splits < 1) splits = 1;
+            // never cut below 128 keys per chunk: the partial state would outweigh the KV it covers
+            const int max_splits = (max_ctx + 127) / 128;
+            if (splits > max_splits) splits = max_splits;
+            if (splits > 64) splits = 64;
+        }
+        pl.chunk_keys = (ceil_div(max_ctx, splits) + 63) / 64 * 64;
+        pl.num_splits = ceil_div(max_ctx, pl.chunk_keys);
+        pl.NS = pl.num_splits + 1;
+        const size_t rows_all = (size_t)pl.B * pl.NS * pl.T_cap * pl.Hq;
+        pl.off_o = 0;
+        pl.off_lse = align_up(rows_all * pl.d * sizeof(float), 256);
+        pl.bytes = pl.off_lse + align_up(rows_all * sizeof(float), 256);
     }
-    int chunk = (ceil_div(max_ctx, splits) + 63) / 64 * 64;
-    pl.chunk_keys = chunk;
-    pl.num_splits = ceil_div(max_ctx, chunk);
-    pl.NS = pl.num_splits + 1;
-    const size_t rows_all = (size_t)pl.B * pl.NS * pl.T_cap * pl.Hq;
-    pl.off_o = 0;
-    pl.off_lse = align_up(rows_all * pl.d * sizeof(float), 256);
-    pl.bytes = pl.off_lse + align_up(rows_all * sizeof(float), 256);
     *out = pl;
     return D2SD_OK;
 }
@@ -172,13 +195,24 @@ int32_t d2sd_cascade_verify_attn(const d2sd_attn_params* p, const void* q, const
     const int phases = p->phases ? p->phases : 7;
     const bool do_prefix = phases & 1, do_tree = phases & 2, do_merge = phases & 4;
     if (pl.use_tc) {
+        a.tree_o = reinterpret_cast<float*>(static_cast<char*>(workspace) + pl.off_tree_o);
+        a.tree_lse = reinterpret_cast<float*>(static_cast<char*>(workspace) + pl.off_tree_lse);
         if (do_prefix)
             if (int32_t st = launch_attn_prefix_tc(pl, a, s)) return st;
-        if (do_tree)
-            if (int32_t st = launch_attn_mma(pl, a, /*prefix=*/false, /*tree=*/true, s)) return st;
-    } else if (do_prefix || do_tree) {
-        if (int32_t st = launch_attn_mma(pl, a, do_prefix, do_tree, s)) return st;
+        if (do_tree) {  // the tree state goes to its own row-layout region: a plan with no prefix chunks
+            AttnPlan tp = pl;
+            tp.num_splits = 0;
+            tp.NS = 1;
+            AttnArgs ta = a;
+            ta.part_o = a.tree_o;
+            ta.part_lse = a.tree_lse;
+            if (int32_t st = launch_attn_mma(tp, ta, /*prefix=*/false, /*tree=*/true, s)) return st;
+        }
+        if (do_merge) return launch_attn_merge_tc(pl, a, s);
+        return D2SD_OK;
     }
+    if (do_prefix || do_tree)
+        if (int32_t st = launch_attn_mma(pl, a, do_prefix, do_tree, s)) return st;
     if (do_merge) return launch_attn_merge(pl, a, s);
     return D2SD_OK;
 }

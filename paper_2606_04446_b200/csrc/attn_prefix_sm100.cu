@@ -1,20 +1,38 @@
 // Stage (c) prefix pass on tcgen05 / TMEM / TMA (sm_100a).  PAPER.md:52, :124, :154.
 //
-// One CTA = (request b, kv head g, context chunk `split`, group of <= 3 query tiles).  Every tree
-// query of every branch and every GQA head of the group is a row of one batched query matrix
-// (row r = t*G + hh), so the chunk's K/V tiles are pulled from HBM into this SM exactly once and are
-// reused by all <= 384 rows:
+// Every tree query of every branch and every GQA head of one kv head is a row of one batched query
+// matrix (row r = t*G + hh), cut into 128-row M tiles; up to three M tiles form an "M group".  The
+// context is cut into `num_splits` chunks.  One work item = (request b, kv head g, M group, chunk)
+// and is served by a PAIR of CTAs (rank 0 / 1) that stream the same K/V chunk:
 //
-//   S[128 x 64]  = Q_m[128 x 128] . K_j^T      tcgen05.mma, A/B from 128B-swizzled SMEM (TMA), D in TMEM
-//   P            = exp2(c*(S - m_run))         softmax warps, one thread per row (TMEM lane), P -> TMEM
-//   O_m[128x128] += P[128 x 64] . V_j[64x128]  tcgen05.mma, A = P from TMEM, B = V (MN-major SMEM)
+//   M tiles in the group   rank 0 computes                rank 1 computes
+//   3                      tile 0 (all key tiles)         tile 1 (all key tiles)
+//                          + tile 2 on even key tiles     + tile 2 on odd key tiles
+//   2                      tile 0                         tile 1
+//   1                      tile 0 on even key tiles       tile 0 on odd key tiles
 //
-// Warp roles (512 threads): warp 0 = TMA producer, warp 1 = MMA issuer (one thread), warp 2 = TMEM
-// allocator, warps 4..15 = three softmax warpgroups, group m owning query tile m for the whole
-// kernel (running max / sum stay in registers).  TMEM: O_0..O_2 at columns 0/128/256, two S/P
-// buffers of 64 columns at 384/448.  The running max is only raised when the new tile maximum
-// exceeds it by more than 2^8 (lazy rescale), in which case the owning softmax warp rescales its O
-// rows in TMEM before the next P.V is issued.
+// so each CTA holds at most two fp32 O accumulators (2 x 128 TMEM columns) and two S/P buffers
+// (2 x 128 columns) -- the whole 512-column TMEM -- and the tensor work of the 3-tile case is split
+// evenly.  Per unit (one M tile x one 128-key tile):
+//
+//   S[128 x 128] = Q_m[128 x 128] . K_j^T    tcgen05.mma, A/B from 128B-swizzled SMEM (TMA), D in TMEM
+//   P            = exp2(c*(S - m_run))       softmax warpgroup, one thread per row (TMEM lane), P -> TMEM
+//   O_m[128x128] += P[128 x 128] . V_j       tcgen05.mma, A = P from TMEM, B = V (MN-major SMEM)
+//
+// N = 128 keys per MMA keeps the tensor pipe MMA-bound (measured: 67 cycles per M128 N128 K16
+// instruction against 64 ideal; N = 64 instructions are issue/SMEM-bound at 54 cycles against 32).
+//
+// Warp roles (384 threads): warp 0 = TMA producer, warp 1 = MMA issuer (one thread), warp 2 = TMEM
+// allocator, warps 4..11 = softmax: two threads per query row (TMEM lane), warps 4..7 on key columns
+// 0..63 and warps 8..11 on columns 64..127 of every S tile, so that two warps per scheduler share
+// the MUFU pipe; the halves exchange row maxima through shared memory.  Running max / sum stay in
+// registers; the running max is only raised when a tile maximum exceeds it by more than 2^8 (lazy
+// rescale), in which case the owning threads rescale their O row in TMEM before the next P.V.
+//
+// Output: one partial state (normalised O fp32, LSE) per (chunk, rank) "slot", transposed through
+// shared memory (XOR-swizzled 16-byte chunks, conflict-free) and written as whole 512-byte rows.
+// Workspace layout (private to this file and the merge kernel below): O [b][slot][g][rows_pad][128]
+// fp32, LSE [b][slot][g][rows_pad].
 #include <cuda.h>
 
 #include "common.cuh"
@@ -24,35 +42,39 @@ namespace {
 
 constexpr int kD = 128;
 constexpr int kTileM = 128;
-constexpr int kTileN = 64;
-constexpr int kMaxMT = 3;
-constexpr int kStages = 4;
-constexpr int kThreads = 512;
+constexpr int kTileN = 128;
+constexpr int kGroupTiles = 3;  // M tiles per M group
+constexpr int kRing = 5;        // ring of K / V tiles (K_j, V_j, K_j+1, ...)
+constexpr int kThreads = 384;
 constexpr uint32_t kQTileBytes = kTileM * kD * 2;   // 32 KiB: [d_hi 2][128 rows][128 B]
-constexpr uint32_t kKvTileBytes = kTileN * kD * 2;  // 16 KiB: [d_hi 2][64 keys][128 B]
-constexpr uint32_t kStageBytes = 2 * kKvTileBytes;
+constexpr uint32_t kKvTileBytes = kTileN * kD * 2;  // 32 KiB: [d_hi 2][128 keys][128 B]
 constexpr uint32_t kOffQ = 0;
-constexpr uint32_t kOffKv = kMaxMT * kQTileBytes;
-constexpr uint32_t kOffBar = kOffKv + kStages * kStageBytes;
-constexpr uint32_t kSmemBytes = kOffBar + 256 + 1024;  // + barriers + alignment slack
+constexpr uint32_t kOffRing = 2 * kQTileBytes;
+constexpr uint32_t kOffBar = kOffRing + kRing * kKvTileBytes;
+constexpr uint32_t kOffX = kOffBar + 256;                 // softmax exchange: fp32 [2][2][128]
+constexpr uint32_t kSmemUsed = kOffX + 2 * 2 * kTileM * 4;
+constexpr uint32_t kSmemBytes = 232448;                   // the whole 227 KiB: kSmemUsed + alignment slack
 constexpr uint32_t kTmemCols = 512;
-constexpr uint32_t kTmemS = 384;  // S/P buffers behind the three O accumulators
+constexpr uint32_t kTmemS = 256;  // two S/P buffers of 128 columns behind the two O accumulators
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kRescaleThreshold = 8.0f;  // log2 units
 
-// barrier slots (8 bytes each) at kOffBar
+// barrier slots (8 bytes each) at kOffBar.  S-ready / P-ready / O-ready exist PER ACCUMULATOR SLOT
+// (phase = unit count of that slot): a parity wait is only sound if the waiter observes every phase,
+// so barriers are never shared between the two softmax warpgroups.
 enum : uint32_t {
-    kBarQFull = 0,
-    kBarKvFull = 1,                      // [kStages]
-    kBarKvEmpty = kBarKvFull + kStages,  // [kStages]
-    // One S-ready / P-ready / O-ready barrier PER QUERY TILE m (phase = key tile j): a parity wait is only
-    // sound if the waiter observes every phase, so barriers are never shared between softmax groups.
-    kBarSFull = kBarKvEmpty + kStages,   // [kMaxMT]
-    kBarPFull = kBarSFull + kMaxMT,      // [kMaxMT]
-    kBarOReady = kBarPFull + kMaxMT,     // [kMaxMT]
-    kNumBars = kBarOReady + kMaxMT,
+    kBarQFull = 0,                     // [2]
+    kBarFull = 2,                      // [kRing]
+    kBarEmpty = kBarFull + kRing,      // [kRing]
+    kBarSFull = kBarEmpty + kRing,     // [2]
+    kBarPFull = kBarSFull + 2,         // [2]
+    kBarODone = kBarPFull + 2,         // [2]
+    kBarAllDone = kBarODone + 2,       // every MMA of the CTA has completed
+    kNumBars = kBarAllDone + 1,
     kTmemSlot = kNumBars  // uint32 written by tcgen05.alloc
 };
+static_assert((kNumBars + 1) * 8 <= 256, "barrier area");
+static_assert(kSmemUsed + 512 <= kSmemBytes, "shared memory budget");
 
 // ---- PTX wrappers -------------------------------------------------------------------------------
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
@@ -106,7 +128,20 @@ __device__ __forceinline__ void tma_load_5d(uint32_t dst, const CUtensorMap* tm,
 __device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* tm) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(tm)) : "memory");
 }
-constexpr uint64_t kEvictFirst = 0x12F0000000000000ull;  // streamed once: KV
+// shared -> global bulk copy (no tensor map: the destination is one contiguous run of rows)
+__device__ __forceinline__ void bulk_store(void* gdst, uint32_t ssrc, uint32_t bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(ssrc), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_commit_wait_read() {
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+}
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void named_bar_sync(uint32_t id, uint32_t threads) {
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
+}
+constexpr uint64_t kEvictFirst = 0x12F0000000000000ull;  // streamed: KV
 constexpr uint64_t kEvictLast = 0x14F0000000000000ull;   // re-read by every chunk CTA of the head: Q
 
 // D[tmem] (+)= A[smem] . B[smem]
@@ -132,37 +167,43 @@ __device__ __forceinline__ void umma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64
 //   K-major  operand: rows of 128 B (64 bf16 along K); 8-row groups SBO = 1024 B apart; LBO unused (1).
 //   MN-major operand: rows of 128 B (64 bf16 along MN); the next 64 along MN is LBO bytes away, the next
 //                     8 along K is SBO = 1024 B away.
+// The start-address field holds (addr >> 4); advancing an operand by `bytes` adds (bytes >> 4).
 __device__ __forceinline__ uint64_t smem_desc(uint32_t addr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
     return (uint64_t)((addr & 0x3FFFFu) >> 4) | ((uint64_t)(lbo_bytes >> 4) << 16) |
            ((uint64_t)(sbo_bytes >> 4) << 32) | (1ull << 46) | (2ull << 61);
 }
 // Instruction descriptor, kind::f16: fp32 accumulate, bf16 x bf16.
-constexpr uint32_t idesc(uint32_t M, uint32_t N, uint32_t b_mn_major) {
+__host__ __device__ constexpr uint32_t idesc(uint32_t M, uint32_t N, uint32_t b_mn_major) {
     return (1u << 4) | (1u << 7) | (1u << 10) | (b_mn_major << 16) | ((N >> 3) << 17) | ((M >> 4) << 24);
 }
-constexpr uint32_t kIdescQK = idesc(kTileM, kTileN, 0);
 constexpr uint32_t kIdescPV = idesc(kTileM, kD, 1);
 
-__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32]) {
-    asm volatile(
-        "tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,"
-        "%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
-        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
-          "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]),
-          "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]),
-          "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
-        : "r"(taddr));
-}
-__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&r)[32]) {
-    asm volatile(
-        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,"
-        "%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31,%32};" ::"r"(taddr),
-        "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]),
-        "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]), "r"(r[16]), "r"(r[17]), "r"(r[18]),
-        "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]), "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]),
-        "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31])
-        : "memory");
-}
+#define D2SD_R32(r, o)                                                                                     \
+    "=r"(r[o + 0]), "=r"(r[o + 1]), "=r"(r[o + 2]), "=r"(r[o + 3]), "=r"(r[o + 4]), "=r"(r[o + 5]),         \
+        "=r"(r[o + 6]), "=r"(r[o + 7]), "=r"(r[o + 8]), "=r"(r[o + 9]), "=r"(r[o + 10]), "=r"(r[o + 11]),   \
+        "=r"(r[o + 12]), "=r"(r[o + 13]), "=r"(r[o + 14]), "=r"(r[o + 15]), "=r"(r[o + 16]), "=r"(r[o + 17]), \
+        "=r"(r[o + 18]), "=r"(r[o + 19]), "=r"(r[o + 20]), "=r"(r[o + 21]), "=r"(r[o + 22]), "=r"(r[o + 23]), \
+        "=r"(r[o + 24]), "=r"(r[o + 25]), "=r"(r[o + 26]), "=r"(r[o + 27]), "=r"(r[o + 28]), "=r"(r[o + 29]), \
+        "=r"(r[o + 30]), "=r"(r[o + 31])
+#define D2SD_W32(r, o)                                                                                     \
+    "r"(r[o + 0]), "r"(r[o + 1]), "r"(r[o + 2]), "r"(r[o + 3]), "r"(r[o + 4]), "r"(r[o + 5]), "r"(r[o + 6]),   \
+        "r"(r[o + 7]), "r"(r[o + 8]), "r"(r[o + 9]), "r"(r[o + 10]), "r"(r[o + 11]), "r"(r[o + 12]),         \
+        "r"(r[o + 13]), "r"(r[o + 14]), "r"(r[o + 15]), "r"(r[o + 16]), "r"(r[o + 17]), "r"(r[o + 18]),      \
+        "r"(r[o + 19]), "r"(r[o + 20]), "r"(r[o + 21]), "r"(r[o + 22]), "r"(r[o + 23]), "r"(r[o + 24]),      \
+        "r"(r[o + 25]), "r"(r[o + 26]), "r"(r[o + 27]), "r"(r[o + 28]), "r"(r[o + 29]), "r"(r[o + 30]),      \
+        "r"(r[o + 31])
+#define D2SD_TMEM_LD32(taddr, r, o)                                                                         \
+    asm volatile(                                                                                           \
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,"    \
+        "%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"                          \
+        : D2SD_R32(r, o)                                                                                    \
+        : "r"(taddr))
+#define D2SD_TMEM_ST32(taddr, r, o)                                                                         \
+    asm volatile(                                                                                           \
+        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15," \
+        "%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31,%32};" ::"r"(taddr),               \
+        D2SD_W32(r, o)                                                                                      \
+        : "memory")
 __device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 
@@ -176,52 +217,91 @@ __device__ __forceinline__ uint32_t pack2_bf16(float lo, float hi) {
     return *reinterpret_cast<uint32_t*>(&v);
 }
 
+// Which accumulator slots of a CTA are live, and on which key tiles the shared slot runs.
+struct SlotPlan {
+    int tile[2];   // M tile (within the M group) of slot 0 (own) / slot 1 (shared), or -1
+    __device__ __forceinline__ bool own() const { return tile[0] >= 0; }
+    __device__ __forceinline__ bool shared_on(int j, int rank) const { return tile[1] >= 0 && (j & 1) == rank; }
+    __device__ __forceinline__ bool used(int j, int rank) const { return own() || shared_on(j, rank); }
+};
+__device__ __forceinline__ SlotPlan make_slots(int MT, int rank) {
+    SlotPlan s;
+    s.tile[0] = MT >= 2 ? rank : -1;
+    s.tile[1] = (MT & 1) ? MT - 1 : -1;
+    return s;
+}
+
+#ifdef D2SD_TIMELINE
+// Debug builds only (-DD2SD_TIMELINE): per-CTA cycle stamps of pipeline events, read back with
+// d2sd_debug_timeline().  Not part of the C ABI.
+__device__ long long g_timeline[256][128];
+#define TL(slot)                                                                                    \
+    do {                                                                                            \
+        const int _c = blockIdx.x + gridDim.x * blockIdx.y;                                         \
+        if (_c < 256 && (slot) < 128) g_timeline[_c][(slot)] = clock64() - tl_t0;                   \
+    } while (0)
+#else
+#define TL(slot) do {} while (0)
+#endif
+
 // -------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kThreads, 1)
 attn_prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
-                      const __grid_constant__ CUtensorMap tm_v, AttnPlan pl, AttnArgs a, int n_mgroups) {
-    extern __shared__ unsigned char smem_raw[];
+                      const __grid_constant__ CUtensorMap tm_v, AttnPlan pl, AttnArgs a) {
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
     const uint32_t smem_raw_u32 = (uint32_t)__cvta_generic_to_shared(smem_raw);
     const uint32_t smem = (smem_raw_u32 + 1023u) & ~1023u;  // 128B swizzle atoms need 1024 B alignment
+    if (smem - smem_raw_u32 + kSmemUsed > kSmemBytes) __trap();
+    unsigned char* smem_gen = smem_raw + (smem - smem_raw_u32);
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int split = blockIdx.x, g = blockIdx.y;
-    const int b = blockIdx.z / n_mgroups, mg = blockIdx.z - b * n_mgroups;
+#ifdef D2SD_TIMELINE
+    const long long tl_t0 = clock64();
+#endif
+    const int rank = blockIdx.x & 1, split = blockIdx.x >> 1, g = blockIdx.y;
+    const int b = blockIdx.z / pl.n_mgroups, mg = blockIdx.z - b * pl.n_mgroups;
     const int G = pl.G;
     const int rows_valid = a.tree_len[b] * G;
-    const int row_base = mg * (kMaxMT * kTileM);
+    const int row_base = mg * (kGroupTiles * kTileM);
     if (row_base >= rows_valid) return;
-    const int MT = min(kMaxMT, (rows_valid - row_base + kTileM - 1) / kTileM);
+    const int MT = min(kGroupTiles, (rows_valid - row_base + kTileM - 1) / kTileM);
+    const SlotPlan sp = make_slots(MT, rank);
     const int L = a.ctx_len[b];
     const int k_begin = split * pl.chunk_keys;
     const int k_end = min(L, k_begin + pl.chunk_keys);
-    float* po = a.part_o + (((size_t)b * pl.NS + split) * pl.T_cap) * pl.Hq * kD;
-    float* plse = a.part_lse + (((size_t)b * pl.NS + split) * pl.T_cap) * pl.Hq;
-    if (k_begin >= k_end) {  // empty chunk: state (O = 0, LSE = -inf); O is never read by the merge
-        for (int r = row_base + tid; r < min(rows_valid, row_base + kMaxMT * kTileM); r += kThreads) {
-            const int t = r / G;
-            plse[(size_t)t * pl.Hq + g * G + (r - t * G)] = -INFINITY;
+    const int slot_id = 2 * split + rank;
+    const size_t slot_row0 = (((size_t)b * pl.NSLOT + slot_id) * pl.Hkv + g) * pl.rows_pad;
+    float* po = a.part_o + slot_row0 * kD;
+    float* plse = a.part_lse + slot_row0;
+    const int n_tiles = k_begin < k_end ? (k_end - k_begin + kTileN - 1) / kTileN : 0;
+    if (n_tiles == 0) {  // empty chunk: state (O = 0, LSE = -inf); O is never read by the merge
+        for (int s = 0; s < 2; ++s) {
+            if (sp.tile[s] < 0) continue;
+            const int r0 = row_base + sp.tile[s] * kTileM;
+            for (int r = r0 + tid; r < min(rows_valid, r0 + kTileM); r += kThreads) plse[r] = -INFINITY;
         }
         return;
     }
-    const int n_tiles = (k_end - k_begin + kTileN - 1) / kTileN;
     const int kv_row0 = (a.kv_indptr ? a.kv_indptr[b] : 0) + k_begin;
+    const int last_valid = (k_end - k_begin) - (n_tiles - 1) * kTileN;  // valid keys of the last key tile
+    const int last_n = (last_valid + 15) & ~15;                         // its MMA N (multiple of 16)
 
     const uint32_t bar0 = smem + kOffBar;
     auto bar = [&](uint32_t i) { return bar0 + 8u * i; };
-    volatile uint32_t* tmem_slot =
-        reinterpret_cast<volatile uint32_t*>(smem_raw + (smem - smem_raw_u32) + kOffBar + 8u * kTmemSlot);
+    volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(smem_gen + kOffBar + 8u * kTmemSlot);
 
     if (warp == 0 && lane == 0) {
-        mbar_init(bar(kBarQFull), 1);
-        for (int s = 0; s < kStages; ++s) {
-            mbar_init(bar(kBarKvFull + s), 1);
-            mbar_init(bar(kBarKvEmpty + s), 1);
+        mbar_init(bar(kBarQFull + 0), 1);
+        mbar_init(bar(kBarQFull + 1), 1);
+        for (int i = 0; i < kRing; ++i) {
+            mbar_init(bar(kBarFull + i), 1);
+            mbar_init(bar(kBarEmpty + i), 1);
         }
-        for (int m = 0; m < kMaxMT; ++m) {
-            mbar_init(bar(kBarSFull + m), 1);
-            mbar_init(bar(kBarPFull + m), kTileM);
-            mbar_init(bar(kBarOReady + m), 1);
+        for (int s = 0; s < 2; ++s) {
+            mbar_init(bar(kBarSFull + s), 1);
+            mbar_init(bar(kBarPFull + s), 2 * kTileM);
+            mbar_init(bar(kBarODone + s), 1);
         }
+        mbar_init(bar(kBarAllDone), 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         tma_prefetch_desc(&tm_q);
         tma_prefetch_desc(&tm_k);
@@ -237,171 +317,353 @@ attn_prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
+    if (tid == 0) TL(0);
 
     if (warp == 0) {
-        // ===== TMA producer =====
+        // ===== TMA producer: K_0 first (the first MMA needs it), then the Q tiles, then the ring =====
         if (lane == 0) {
-            mbar_expect_tx(bar(kBarQFull), MT * kQTileBytes);
-            for (int m = 0; m < MT; ++m) {
-                const int t0 = b * pl.T_cap + (row_base + m * kTileM) / G;
-                tma_load_5d(smem + kOffQ + m * kQTileBytes, &tm_q, bar(kBarQFull), 0, 0, t0, 0, g, kEvictLast);
-            }
+            int x = 0;  // ring position of the next tile to load
+            bool q_sent = false;
             for (int j = 0; j < n_tiles; ++j) {
-                const int s = j % kStages;
-                mbar_wait(bar(kBarKvEmpty + s), ((j / kStages) & 1) ^ 1);
-                mbar_expect_tx(bar(kBarKvFull + s), kStageBytes);
-                const uint32_t dst = smem + kOffKv + s * kStageBytes;
-                tma_load_4d(dst, &tm_k, bar(kBarKvFull + s), 0, kv_row0 + j * kTileN, 0, g, kEvictFirst);
-                tma_load_4d(dst + kKvTileBytes, &tm_v, bar(kBarKvFull + s), 0, kv_row0 + j * kTileN, 0, g, kEvictFirst);
+                if (!sp.used(j, rank)) continue;
+                for (int kv = 0; kv < 2; ++kv, ++x) {
+                    const int i = x % kRing;
+                    mbar_wait(bar(kBarEmpty + i), ((x / kRing) & 1) ^ 1);
+                    mbar_expect_tx(bar(kBarFull + i), kKvTileBytes);
+                    tma_load_4d(smem + kOffRing + i * kKvTileBytes, kv ? &tm_v : &tm_k, bar(kBarFull + i), 0,
+                                kv_row0 + j * kTileN, 0, g, kEvictFirst);
+                    if (!q_sent) {
+                        q_sent = true;
+                        for (int s = 0; s < 2; ++s) {
+                            if (sp.tile[s] < 0) continue;
+                            const int t0 = b * pl.T_cap + (row_base + sp.tile[s] * kTileM) / G;
+                            mbar_expect_tx(bar(kBarQFull + s), kQTileBytes);
+                            tma_load_5d(smem + kOffQ + s * kQTileBytes, &tm_q, bar(kBarQFull + s), 0, 0, t0, 0, g,
+                                        kEvictLast);
+                        }
+                    }
+                }
             }
         }
     } else if (warp == 1) {
-        // ===== MMA issuer (one thread) =====
+        // ===== MMA issuer (one thread).  Issue order: QK(n+1) before PV(n), so that the tensor pipe
+        // works on the next S while the softmax warpgroup turns S_n into P_n. =====
         if (lane == 0) {
-            const int U = n_tiles * MT;
-            mbar_wait(bar(kBarQFull), 0);
-            for (int u = 0; u <= U; ++u) {
-                if (u < U) {  // S_u = Q_m K_j^T into S buffer u&1
-                    const int j = u / MT, m = u - j * MT, s = j % kStages;
-                    if (m == 0) mbar_wait(bar(kBarKvFull + s), (j / kStages) & 1);
+            const uint64_t qd[2] = {smem_desc(smem + kOffQ, 16, 1024), smem_desc(smem + kOffQ + kQTileBytes, 16, 1024)};
+            int n = 0, x = 0;
+            int cnt_qk[2] = {0, 0}, cnt_pv[2] = {0, 0};
+            // the PV that is still owed (unit n-1)
+            bool pend = false, pend_last = false;
+            int pend_slot = 0, pend_sbuf = 0, pend_vx = 0, pend_n = 0;
+            bool v_waited = false;
+            auto do_pv = [&]() {
+                const int s = pend_slot, vi = pend_vx % kRing;
+                mbar_wait(bar(kBarPFull + s), cnt_pv[s] & 1);
+                if (!v_waited) {
+                    mbar_wait(bar(kBarFull + vi), (pend_vx / kRing) & 1);
+                    v_waited = true;
+                }
+                tc_fence_after();
+                const uint64_t vd = smem_desc(smem + kOffRing + vi * kKvTileBytes, kKvTileBytes / 2, 1024);
+                const uint32_t pa = tmem + kTmemS + pend_sbuf * kTileN;
+                const uint32_t od = tmem + s * kD;
+                const int ksteps = pend_n >> 4;
+#pragma unroll 1
+                for (int ks = 0; ks < ksteps; ++ks)
+                    umma_ts(od, pa + ks * 8, vd + (uint64_t)(ks * (2048 >> 4)), kIdescPV, (cnt_pv[s] | ks) != 0);
+                tc_commit(bar(kBarODone + s));
+                if (pend_last) tc_commit(bar(kBarEmpty + vi));
+                ++cnt_pv[s];
+                pend = false;
+            };
+            for (int j = 0; j < n_tiles; ++j) {
+                if (!sp.used(j, rank)) continue;
+                const int kx = x, vx = x + 1;
+                x += 2;
+                const int ki = kx % kRing;
+                const int tile_n = (j == n_tiles - 1) ? last_n : kTileN;
+                const bool sh = sp.shared_on(j, rank);
+                mbar_wait(bar(kBarFull + ki), (kx / kRing) & 1);
+                const uint64_t kd = smem_desc(smem + kOffRing + ki * kKvTileBytes, 16, 1024);
+                const uint32_t id_qk = idesc(kTileM, (uint32_t)tile_n, 0);
+                for (int s = 0; s < 2; ++s) {
+                    if (s == 0 ? !sp.own() : !sh) continue;
+                    const bool last_of_tile = (s == 1) || !sh;
+                    if (cnt_qk[s] == 0) mbar_wait(bar(kBarQFull + s), 0);
+                    TL(16 + 3 * n);
                     tc_fence_after();
-                    const uint32_t qa = smem + kOffQ + m * kQTileBytes;
-                    const uint32_t ka = smem + kOffKv + s * kStageBytes;
+                    const uint32_t sd = tmem + kTmemS + (n & 1) * kTileN;
 #pragma unroll
                     for (int kk = 0; kk < kD / 16; ++kk) {
-                        const uint64_t ad = smem_desc(qa + (kk >> 2) * (kQTileBytes / 2) + (kk & 3) * 32, 16, 1024);
-                        const uint64_t bd = smem_desc(ka + (kk >> 2) * (kKvTileBytes / 2) + (kk & 3) * 32, 16, 1024);
-                        umma_ss(tmem + kTmemS + (u & 1) * kTileN, ad, bd, kIdescQK, kk > 0);
+                        const uint64_t off = (uint64_t)(((kk >> 2) * (kQTileBytes / 2) + (kk & 3) * 32) >> 4);
+                        umma_ss(sd, qd[s] + off, kd + off, id_qk, kk > 0);
                     }
-                    tc_commit(bar(kBarSFull + m));
-                }
-                if (u >= 1) {  // O_m += P_v V_j, P read from TMEM (aliases S buffer v&1)
-                    const int v = u - 1;
-                    const int j = v / MT, m = v - j * MT, s = j % kStages;
-                    mbar_wait(bar(kBarPFull + m), j & 1);
-                    tc_fence_after();
-                    const uint32_t va = smem + kOffKv + s * kStageBytes + kKvTileBytes;
-#pragma unroll
-                    for (int kk = 0; kk < kTileN / 16; ++kk) {
-                        const uint64_t bd = smem_desc(va + kk * 2048, kKvTileBytes / 2, 1024);
-                        umma_ts(tmem + m * kD, tmem + kTmemS + (v & 1) * kTileN + kk * 8, bd, kIdescPV,
-                                (j > 0 || kk > 0));
+                    tc_commit(bar(kBarSFull + s));
+                    if (last_of_tile) tc_commit(bar(kBarEmpty + ki));
+                    ++cnt_qk[s];
+                    if (pend) {
+                        do_pv();
+                        TL(16 + 3 * (n - 1) + 2);
                     }
-                    tc_commit(bar(kBarOReady + m));
-                    if (m == MT - 1) tc_commit(bar(kBarKvEmpty + s));
+                    pend = true; pend_slot = s; pend_sbuf = n & 1; pend_vx = vx; pend_n = tile_n;
+                    pend_last = last_of_tile;
+                    if (s == 0 || !sp.own()) v_waited = false;  // first unit of this key tile: V_j not yet waited for
+                    ++n;
                 }
             }
+            if (pend) do_pv();
+            tc_commit(bar(kBarAllDone));
         }
     } else if (warp >= 4) {
-        // ===== softmax warpgroup m: one thread per query row =====
-        const int m = (warp - 4) >> 2;
-        if (m < MT) {
-            const int w = warp & 3;
-            const int r = row_base + m * kTileM + w * 32 + lane;  // this thread's row
-            const bool warp_active = (row_base + m * kTileM + w * 32) < rows_valid;
-            const uint32_t lane_addr = (uint32_t)(w * 32) << 16;
-            const float c2 = pl.sm_scale * kLog2e;
-            const float thr = kRescaleThreshold / c2;  // in raw score units
-            float m_run = -INFINITY, l_run = 0.f;
-            for (int j = 0; j < n_tiles; ++j) {
-                const int u = j * MT + m;
-                const uint32_t sbuf = tmem + kTmemS + (u & 1) * kTileN + lane_addr;
-                mbar_wait(bar(kBarSFull + m), j & 1);
-                bool saw_o = false;  // every phase of O-ready must be observed (parity waits)
+        // ===== softmax: warps 4..7 take key columns 0..63 of every S tile, warps 8..11 columns 64..127;
+        // thread (w, lane) of either half owns query row w*32 + lane (TMEM lane).  The two halves
+        // exchange their row maxima through shared memory once per unit. =====
+        const int h = (warp - 4) >> 2;
+        const int w = warp & 3;
+        const int rl = w * 32 + lane;  // row within the tile
+        const uint32_t lane_addr = (uint32_t)(w * 32) << 16;
+        const float c2 = pl.sm_scale * kLog2e;
+        const float thr = kRescaleThreshold / c2;  // in raw score units
+        float* xm = reinterpret_cast<float*>(smem_gen + kOffX);  // [2 unit parity][2 halves][128 rows]
+        float m_run[2] = {-INFINITY, -INFINITY}, l_run[2] = {0.f, 0.f};
+        int kcnt[2] = {0, 0};
+        int n = 0;
+        for (int j = 0; j < n_tiles; ++j) {
+            if (!sp.used(j, rank)) continue;
+            const bool sh = sp.shared_on(j, rank);
+            const bool last_tile = (j == n_tiles - 1) && last_valid < kTileN;
+#pragma unroll
+            for (int s = 0; s < 2; ++s) {
+                if (s == 0 ? !sp.own() : !sh) continue;
+                const int k = kcnt[s];
+                const bool warp_active = (row_base + sp.tile[s] * kTileM + w * 32) < rows_valid;
+                const uint32_t sbuf = tmem + kTmemS + (n & 1) * kTileN + lane_addr;
+                const uint32_t o_addr = tmem + s * kD + h * 64 + lane_addr;
+                mbar_wait(bar(kBarSFull + s), k & 1);
+                if (warp == 4 && lane == 0) TL(64 + 2 * n);
+                uint32_t sv[64];
+                float mxh = -INFINITY;
                 if (warp_active) {
                     tc_fence_after();
-                    uint32_t s0[32], s1[32];
-                    tmem_ld32(sbuf, s0);
-                    tmem_ld32(sbuf + 32, s1);
+                    D2SD_TMEM_LD32(sbuf + h * 64, sv, 0);
+                    D2SD_TMEM_LD32(sbuf + h * 64 + 32, sv, 32);
                     tmem_wait_ld();
-                    const int valid = k_end - (k_begin + j * kTileN);  // keys of this tile inside the chunk
-                    if (valid < kTileN) {
+                    if (last_tile) {
 #pragma unroll
-                        for (int c = 0; c < 32; ++c) {
-                            if (c >= valid) s0[c] = 0xFF800000u;       // -inf
-                            if (c + 32 >= valid) s1[c] = 0xFF800000u;
-                        }
+                        for (int c = 0; c < 64; ++c)
+                            if (h * 64 + c >= last_valid) sv[c] = 0xFF800000u;  // -inf: keys outside the chunk
                     }
-                    float mx = -INFINITY;
+                    float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;
 #pragma unroll
-                    for (int c = 0; c < 32; ++c) mx = fmaxf(mx, fmaxf(__uint_as_float(s0[c]), __uint_as_float(s1[c])));
+                    for (int c = 0; c < 64; c += 4) {
+                        mx0 = fmaxf(mx0, __uint_as_float(sv[c]));
+                        mx1 = fmaxf(mx1, __uint_as_float(sv[c + 1]));
+                        mx2 = fmaxf(mx2, __uint_as_float(sv[c + 2]));
+                        mx3 = fmaxf(mx3, __uint_as_float(sv[c + 3]));
+                    }
+                    mxh = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
+                }
+                xm[((n & 1) * 2 + h) * kTileM + rl] = mxh;
+                named_bar_sync(1, 256);  // also orders "both halves have read S" before "P overwrites S"
+                bool saw_o = false;      // every phase of O-done must be observed (parity waits)
+                if (warp_active) {
+                    const float mx = fmaxf(mxh, xm[((n & 1) * 2 + (h ^ 1)) * kTileM + rl]);
                     // lazy rescale: raise the running max only when it is exceeded by more than 2^8
-                    const bool need = mx > m_run + thr;
-                    if (j == 0) {
-                        m_run = mx;
+                    const bool need = mx > m_run[s] + thr;
+                    if (k == 0) {
+                        m_run[s] = mx;
                     } else if (__any_sync(0xffffffffu, need)) {
-                        const float alpha = need ? ex2((m_run - mx) * c2) : 1.f;
-                        mbar_wait(bar(kBarOReady + m), (j - 1) & 1);  // previous P.V into O_m has landed
+                        const float alpha = need ? ex2((m_run[s] - mx) * c2) : 1.f;
+                        mbar_wait(bar(kBarODone + s), (k - 1) & 1);  // previous P.V into this O has landed
                         saw_o = true;
                         tc_fence_after();
 #pragma unroll 1
-                        for (int c0 = 0; c0 < kD; c0 += 32) {
+                        for (int c0 = 0; c0 < 64; c0 += 32) {  // this half's 64 of the 128 O columns
                             uint32_t o[32];
-                            tmem_ld32(tmem + m * kD + c0 + lane_addr, o);
+                            D2SD_TMEM_LD32(o_addr + c0, o, 0);
                             tmem_wait_ld();
 #pragma unroll
                             for (int c = 0; c < 32; ++c) o[c] = __float_as_uint(__uint_as_float(o[c]) * alpha);
-                            tmem_st32(tmem + m * kD + c0 + lane_addr, o);
+                            D2SD_TMEM_ST32(o_addr + c0, o, 0);
                         }
                         tmem_wait_st();
                         if (need) {
-                            m_run = mx;
-                            l_run *= alpha;
+                            m_run[s] = mx;
+                            l_run[s] *= alpha;
                         }
                     }
-                    const float ms = m_run * c2;
-                    float sum = 0.f;
+                    const float ms = m_run[s] * c2;
+                    float sum0 = 0.f, sum1 = 0.f;
                     uint32_t p[32];
 #pragma unroll
-                    for (int c = 0; c < 16; ++c) {
-                        const float e0 = ex2(__uint_as_float(s0[2 * c]) * c2 - ms);
-                        const float e1 = ex2(__uint_as_float(s0[2 * c + 1]) * c2 - ms);
-                        const float e2 = ex2(__uint_as_float(s1[2 * c]) * c2 - ms);
-                        const float e3 = ex2(__uint_as_float(s1[2 * c + 1]) * c2 - ms);
-                        sum += (e0 + e1) + (e2 + e3);
+                    for (int c = 0; c < 32; c += 2) {
+                        const float e0 = ex2(__uint_as_float(sv[2 * c]) * c2 - ms);
+                        const float e1 = ex2(__uint_as_float(sv[2 * c + 1]) * c2 - ms);
+                        const float e2 = ex2(__uint_as_float(sv[2 * c + 2]) * c2 - ms);
+                        const float e3 = ex2(__uint_as_float(sv[2 * c + 3]) * c2 - ms);
+                        sum0 += e0 + e1;
+                        sum1 += e2 + e3;
                         p[c] = pack2_bf16(e0, e1);
-                        p[16 + c] = pack2_bf16(e2, e3);
+                        p[c + 1] = pack2_bf16(e2, e3);
                     }
-                    l_run += sum;
-                    tmem_st32(sbuf, p);  // P[128 x 64] bf16 = 32 columns, K contiguous, 2 per column
+                    l_run[s] += sum0 + sum1;
+                    // P[128 x 128] bf16 = 64 columns (2 keys per column): this half writes columns 32h..32h+31
+                    D2SD_TMEM_ST32(sbuf + h * 32, p, 0);
                     tmem_wait_st();
                     tc_fence_before();
                 }
-                mbar_arrive(bar(kBarPFull + m));
-                if (j > 0 && !saw_o) mbar_wait(bar(kBarOReady + m), (j - 1) & 1);
-            }
-            // epilogue: O_m / l -> partial state of this chunk
-            mbar_wait(bar(kBarOReady + m), (n_tiles - 1) & 1);
-            if (warp_active) {
-                tc_fence_after();
-                const bool row_ok = r < rows_valid;
-                const int t = r / G;
-                const int h = g * G + (r - t * G);
-                const float inv = 1.f / l_run;
-                float* orow = po + ((size_t)t * pl.Hq + h) * kD;
-#pragma unroll 1
-                for (int c0 = 0; c0 < kD; c0 += 32) {
-                    uint32_t o[32];
-                    tmem_ld32(tmem + m * kD + c0 + lane_addr, o);
-                    tmem_wait_ld();
-                    if (row_ok) {
-#pragma unroll
-                        for (int c = 0; c < 32; c += 4)
-                            *reinterpret_cast<float4*>(orow + c0 + c) =
-                                make_float4(__uint_as_float(o[c]) * inv, __uint_as_float(o[c + 1]) * inv,
-                                            __uint_as_float(o[c + 2]) * inv, __uint_as_float(o[c + 3]) * inv);
-                    }
-                }
-                if (row_ok) plse[(size_t)t * pl.Hq + h] = m_run * pl.sm_scale + logf(l_run);
+                mbar_arrive(bar(kBarPFull + s));
+                if (warp == 4 && lane == 0) TL(64 + 2 * n + 1);
+                if (k > 0 && !saw_o) mbar_wait(bar(kBarODone + s), (k - 1) & 1);
+                ++kcnt[s];
+                ++n;
             }
         }
+        // ---- epilogue: O / l -> shared staging -> coalesced stores of the slot's partial state ----
+        mbar_wait(bar(kBarAllDone), 0);  // every MMA done: the ring is free for staging
+        if (warp == 4 && lane == 0) TL(100);
+#pragma unroll
+        for (int s = 0; s < 2; ++s) {
+            if (sp.tile[s] < 0) continue;
+            const int tile_row0 = row_base + sp.tile[s] * kTileM;
+            const int r = tile_row0 + rl;
+            const bool row_ok = r < rows_valid;
+            if (kcnt[s] == 0) {  // this rank had no unit for the slot (shared tile, single key tile)
+                if (h == 0 && row_ok) plse[r] = -INFINITY;
+                continue;
+            }
+            const bool warp_active = (tile_row0 + w * 32) < rows_valid;
+            xm[h * kTileM + rl] = l_run[s];
+            named_bar_sync(1, 256);
+            const float l_tot = l_run[s] + xm[(h ^ 1) * kTileM + rl];
+            const uint32_t stage = smem + kOffRing + (uint32_t)s * (2 * kKvTileBytes);
+            if (warp_active) {
+                tc_fence_after();
+                const float inv = 1.f / l_tot;
+                const uint32_t srow = stage + (uint32_t)rl * 512u;
+                const uint32_t o_addr = tmem + s * kD + h * 64 + lane_addr;
+#pragma unroll
+                for (int c0 = 0; c0 < 64; c0 += 32) {
+                    uint32_t o[32];
+                    D2SD_TMEM_LD32(o_addr + c0, o, 0);
+                    tmem_wait_ld();
+#pragma unroll
+                    for (int c = 0; c < 32; c += 4) {
+                        const uint32_t chunk = (uint32_t)((h * 64 + c0 + c) >> 2);
+                        const uint32_t phys = (chunk & ~7u) | ((chunk ^ (uint32_t)rl) & 7u);
+                        asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(srow + phys * 16u),
+                                     "f"(__uint_as_float(o[c]) * inv), "f"(__uint_as_float(o[c + 1]) * inv),
+                                     "f"(__uint_as_float(o[c + 2]) * inv), "f"(__uint_as_float(o[c + 3]) * inv)
+                                     : "memory");
+                    }
+                }
+                if (h == 0 && row_ok) plse[r] = m_run[s] * pl.sm_scale + logf(l_tot);
+            }
+            named_bar_sync(1, 256);
+            // warp q of the eight stores rows q*16 .. q*16+15, one 512-byte row per instruction
+            const int nrows = min(kTileM, rows_valid - tile_row0);
+            const int q = warp - 4;
+            const uint32_t chunk = (uint32_t)lane;
+#pragma unroll 4
+            for (int i = 0; i < 16; ++i) {
+                const int row = q * 16 + i;
+                if (row < nrows) {
+                    const uint32_t phys = (chunk & ~7u) | ((chunk ^ (uint32_t)row) & 7u);
+                    float4 v;
+                    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];"
+                                 : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
+                                 : "r"(stage + (uint32_t)row * 512u + phys * 16u));
+                    *reinterpret_cast<float4*>(po + (size_t)(tile_row0 + row) * kD + lane * 4) = v;
+                }
+            }
+        }
+        if (warp == 4 && lane == 0) TL(101);
     }
 
     tc_fence_before();
     __syncthreads();
+    if (tid == 0) TL(2);
     if (warp == 2) {
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(kTmemCols) : "memory");
     }
+}
+
+// Merge for the tcgen05 path: LSE = log sum_p e^{LSE_p};  O = sum_p e^{LSE_p - LSE} O_p over the slots
+// that hold the row's M tile and the tree state ("cascade attention" state merge).
+// One warp per (b,t,h) row; lane i first fetches the LSE of relevant slot i, then the warp sweeps
+// the slots' O rows (512 B each, coalesced).
+__global__ void __launch_bounds__(128) attn_merge_tc_kernel(AttnPlan pl, AttnArgs a) {
+    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    const int rows_per_req = pl.T_cap * pl.Hq;
+    if (warp >= pl.B * rows_per_req) return;
+    const int b = warp / rows_per_req;
+    const int th = warp - b * rows_per_req;  // t*Hq + h
+    const int t = th / pl.Hq, h = th - t * pl.Hq;
+    const int T = a.tree_len[b];
+    if (t >= T) return;
+    const int G = pl.G, g = h / G;
+    const int r = t * G + (h - g * G);
+    const int mg = r / (kGroupTiles * kTileM);
+    const int tl = (r - mg * kGroupTiles * kTileM) / kTileM;
+    const int MT = min(kGroupTiles, (T * G - mg * kGroupTiles * kTileM + kTileM - 1) / kTileM);
+    const bool own = MT >= 2 && tl < 2;       // tile owned by rank tl; otherwise shared by both ranks
+    const int n_rel = own ? pl.num_splits : 2 * pl.num_splits;  // relevant slots (<= 128)
+    auto slot_of = [&](int i) { return own ? 2 * i + tl : i; };
+    auto row_of = [&](int slot) { return (((size_t)b * pl.NSLOT + slot) * pl.Hkv + g) * pl.rows_pad + r; };
+
+    float m = -INFINITY, wsum = 0.f;
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int base = 0; base < n_rel; base += 32) {
+        const int i = base + lane;
+        const float l = i < n_rel ? a.part_lse[row_of(slot_of(i))] : -INFINITY;
+        float mb = l;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) mb = fmaxf(mb, __shfl_xor_sync(0xffffffffu, mb, o));
+        if (mb == -INFINITY) continue;
+        if (mb > m) {  // rescale what has been accumulated so far (only with > 32 relevant slots)
+            const float sc = m == -INFINITY ? 0.f : __expf(m - mb);
+            acc.x *= sc; acc.y *= sc; acc.z *= sc; acc.w *= sc;
+            wsum *= sc;
+            m = mb;
+        }
+        const float wl = l == -INFINITY ? 0.f : __expf(l - m);
+        const int cnt = min(32, n_rel - base);
+#pragma unroll 4
+        for (int q = 0; q < cnt; ++q) {
+            const float w = __shfl_sync(0xffffffffu, wl, q);
+            if (w == 0.f) continue;
+            const float4 o = *reinterpret_cast<const float4*>(a.part_o + row_of(slot_of(base + q)) * kD + lane * 4);
+            wsum += w;
+            acc.x += w * o.x; acc.y += w * o.y; acc.z += w * o.z; acc.w += w * o.w;
+        }
+    }
+    const float lse_prefix = (m > -INFINITY) ? m + logf(wsum) : -INFINITY;
+    const float lt = a.tree_lse[(size_t)b * rows_per_req + th];
+    const float4 ot = *reinterpret_cast<const float4*>(a.tree_o + ((size_t)b * rows_per_req + th) * kD + lane * 4);
+    if (a.dbg_state) {
+        const size_t rs = (size_t)(kD + 1);
+        float* d0 = a.dbg_state + ((size_t)b * rows_per_req + th) * rs;
+        float* d1 = d0 + (size_t)pl.B * rows_per_req * rs;
+        const float inv = wsum > 0.f ? 1.f / wsum : 0.f;
+        d0[lane * 4 + 0] = acc.x * inv; d0[lane * 4 + 1] = acc.y * inv;
+        d0[lane * 4 + 2] = acc.z * inv; d0[lane * 4 + 3] = acc.w * inv;
+        d1[lane * 4 + 0] = ot.x; d1[lane * 4 + 1] = ot.y; d1[lane * 4 + 2] = ot.z; d1[lane * 4 + 3] = ot.w;
+        if (lane == 0) { d0[kD] = lse_prefix; d1[kD] = lt; }
+    }
+    // fold the tree state in (lt is finite: every row has its self bit)
+    const float m2 = fmaxf(m, lt);
+    const float sp = (m > -INFINITY) ? __expf(m - m2) : 0.f;
+    const float wt = __expf(lt - m2);
+    const float tot = wsum * sp + wt;
+    const float inv = 1.f / tot;
+    const float ox = (acc.x * sp + wt * ot.x) * inv, oy = (acc.y * sp + wt * ot.y) * inv;
+    const float oz = (acc.z * sp + wt * ot.z) * inv, ow = (acc.w * sp + wt * ot.w) * inv;
+    __nv_bfloat162 lo = __floats2bfloat162_rn(ox, oy), hi = __floats2bfloat162_rn(oz, ow);
+    uint2 pk;
+    pk.x = *reinterpret_cast<uint32_t*>(&lo);
+    pk.y = *reinterpret_cast<uint32_t*>(&hi);
+    *reinterpret_cast<uint2*>(a.out + ((size_t)b * rows_per_req + th) * kD + lane * 4) = pk;
+    if (a.lse && lane == 0) a.lse[(size_t)b * rows_per_req + th] = m2 + logf(tot);
 }
 
 // ---- host side ----------------------------------------------------------------------------------
@@ -456,18 +718,30 @@ int32_t launch_attn_prefix_tc(const AttnPlan& pl, const AttnArgs& a, cudaStream_
         const cuuint32_t box[5] = {64, (cuuint32_t)pl.G, (cuuint32_t)(kTileM / pl.G), 2, 1};
         if (int32_t st = encode(&tm_q, a.q, 5, dims, strides, box, "q")) return st;
     }
-    {   // K/V [kv_rows, Hkv, d] viewed as (d_lo 64, row, d_hi 2, g): one box = one 64-key tile
+    {   // K/V [kv_rows, Hkv, d] viewed as (d_lo 64, row, d_hi 2, g): one box = one 128-key tile
         const cuuint64_t dims[4] = {64, (cuuint64_t)pl.kv_rows, 2, (cuuint64_t)pl.Hkv};
         const cuuint64_t strides[3] = {(cuuint64_t)pl.Hkv * kD * 2, 128, (cuuint64_t)kD * 2};
         const cuuint32_t box[4] = {64, kTileN, 2, 1};
         if (int32_t st = encode(&tm_k, a.k_cache, 4, dims, strides, box, "k_cache")) return st;
         if (int32_t st = encode(&tm_v, a.v_cache, 4, dims, strides, box, "v_cache")) return st;
     }
-    const int n_mgroups = ceil_div(pl.T_cap * pl.G, kMaxMT * kTileM);
-    dim3 grid(pl.num_splits, pl.Hkv, pl.B * n_mgroups);
-    attn_prefix_tc_kernel<<<grid, kThreads, kSmemBytes, s>>>(tm_q, tm_k, tm_v, pl, a, n_mgroups);
+    dim3 grid(2 * pl.num_splits, pl.Hkv, pl.B * pl.n_mgroups);
+    attn_prefix_tc_kernel<<<grid, kThreads, kSmemBytes, s>>>(tm_q, tm_k, tm_v, pl, a);
     D2SD_CHECK_LAUNCH("attn_prefix_tc_kernel");
     return D2SD_OK;
 }
+
+int32_t launch_attn_merge_tc(const AttnPlan& pl, const AttnArgs& a, cudaStream_t s) {
+    const int rows = pl.B * pl.T_cap * pl.Hq;
+    attn_merge_tc_kernel<<<ceil_div(rows, 4), 128, 0, s>>>(pl, a);
+    D2SD_CHECK_LAUNCH("attn_merge_tc_kernel");
+    return D2SD_OK;
+}
+
+#ifdef D2SD_TIMELINE
+extern "C" int32_t d2sd_debug_timeline(long long* host_buf /* [256][128] */) {
+    return cudaMemcpyFromSymbol(host_buf, g_timeline, sizeof(long long) * 256 * 128) == cudaSuccess ? 0 : -4;
+}
+#endif
 
 }  // namespace d2sd
