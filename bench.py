@@ -8,7 +8,7 @@ synthetic input shaped like BASELINE.json config 2 (Qwen3-8B verification step, 
 K=4, 36 layers with distinct KV, vocab 151936).  `value` = tree tokens verified per second with all
 inputs resident in HBM (CUDA-graph replay of the step, CUDA events, max over ranks); `e2e` = the
 same through the C-ABI binding with HOST (pinned) buffers and the copies inside the timed region;
-`roofline` = the dominant kernel (prefix pass) against the measured peaks; `cpu_baseline` = the CPU
+`roofline` = the dominant kernel (the cascade attention launch) against the measured peaks; `cpu_baseline` = the CPU
 oracle timed on this box's host cores on a bounded sample.  N>1: independent replicas, one per
 rank, no data-path collective ("replicas only").
 """
@@ -208,9 +208,8 @@ class Workload:
 
         B, T, Hq, Hkv, d = cfg.B, cfg.T_cap, cfg.Hq, cfg.Hkv, cfg.d
         kv_rows = self.layers[0]["k_cache"].shape[0] * (cfg.page_size if cfg.paged else 1)
-        self.ws_attn = torch.empty(d2sd.cascade_workspace_bytes(B, T, Hq, Hkv, d, self.max_ctx,
-                                                                page_size=self.page_size, kv_rows=kv_rows),
-                                   dtype=torch.uint8, device=dev)
+        self.ws_attn = d2sd.cascade_workspace(B, T, Hq, Hkv, d, self.max_ctx, device=dev,
+                                              page_size=self.page_size, kv_rows=kv_rows)
         self.ws_acc = torch.empty(d2sd.accept_workspace_bytes(B, T, cfg.V), dtype=torch.uint8, device=dev)
         self.prefix_len = torch.empty((B, cfg.K), dtype=torch.int32, device=dev)
         self.tree = None
@@ -257,11 +256,15 @@ class Workload:
             self.attention(layer)
         self.accept()
 
-    LAUNCHES_PER_LAYER = 3  # prefix pass, tree pass, merge
+    @property
+    def attn_kernel(self) -> str:
+        return "attn_mma_kernel" if self.cfg.paged else "attn_cascade_tc_kernel"
 
     @property
     def launches_per_step(self) -> int:
-        return 2 + self.LAUNCHES_PER_LAYER * self.cfg.layers + 2
+        # select, build, per layer: one fused tcgen05 launch (contiguous KV) or mma.sync pass + merge
+        # (paged KV), argmax, walk
+        return 2 + (2 if self.cfg.paged else 1) * self.cfg.layers + 2
 
     # --- e2e: host buffers in, host results out ---------------------------------------------------
     def h2d_bytes(self, with_kv: bool) -> int:
@@ -421,8 +424,7 @@ def main():
         flush = lambda: fbuf.fill_(1)  # noqa: E731
 
     g_step = capture(torch, wl.step)
-    g_prefix = capture(torch, lambda: [wl.attention(i, phases=1) for i in range(cfg.layers)])
-    wl.step()  # leave consistent state after the prefix-only capture
+    g_attn = capture(torch, lambda: [wl.attention(i) for i in range(cfg.layers)])
 
     clocks = ClockSampler(local)
     for _ in range(args.warmup):
@@ -431,11 +433,12 @@ def main():
     clocks.start()
     ms = time_replays(torch, g_step, args.steps, flush)
     _barrier()
-    # dominant kernel (prefix pass) alone: same launch configuration, same distinct-per-layer KV
+    # dominant kernel (the cascade attention launch) alone: same launch configuration, same
+    # distinct-per-layer KV, back to back as in the step
     for _ in range(3):
-        g_prefix.replay()
+        g_attn.replay()
     torch.cuda.synchronize()
-    ms_prefix = time_replays(torch, g_prefix, args.steps, flush)
+    ms_prefix = time_replays(torch, g_attn, args.steps, flush)
     clocks.stop()
     ms = max_over_ranks(ms)
     tokens_all = sum_over_ranks(float(wl.tree_tokens))
@@ -444,21 +447,22 @@ def main():
 
     # roofline of the prefix pass (algorithmic bytes and flops per launch)
     T_rows = wl.tree_tokens  # tree nodes over all requests
-    q_bytes = T_rows * cfg.Hq * cfg.d * 2
-    alg_bytes = kv_bytes_layer + q_bytes
+    q_bytes = T_rows * cfg.Hq * cfg.d * 2                     # Q in; O out is the same size
+    tree_kv_bytes = 2 * T_rows * cfg.Hkv * cfg.d * 2
+    alg_bytes = kv_bytes_layer + 2 * q_bytes + tree_kv_bytes + T_rows * cfg.Hq * 4
     alg_flops = 4.0 * cfg.Hq * cfg.d * float(sum(int(t) * int(l) for t, l in zip(wl.tree_len_host, wl.st["ctx_len"])))
     us_prefix = ms_prefix / (args.steps * cfg.layers) * 1e3
     t_hbm_us = alg_bytes / (peaks["hbm_gbs"] * 1e9) * 1e6
     t_tc_us = alg_flops / (peaks["bf16_tflops_sustained"] * 1e12) * 1e6
     ach_gbs = alg_bytes / (us_prefix * 1e-6) / 1e9
     ach_tf = alg_flops / (us_prefix * 1e-6) / 1e12
-    traffic = ncu_traffic("prefix", cfg.number)
+    traffic = ncu_traffic(wl.attn_kernel, cfg.number)
     roof_hbm = {"bound": "hbm", "achieved": ach_gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                 "frac": ach_gbs / peaks["hbm_gbs"], "traffic": traffic, "peak_source": peaks["source"],
-                "kernel": "prefix pass", "us_per_launch": us_prefix, "alg_bytes_per_launch": alg_bytes}
+                "kernel": wl.attn_kernel, "us_per_launch": us_prefix, "alg_bytes_per_launch": alg_bytes}
     roof_tc = {"bound": "tensor", "achieved": ach_tf, "peak": peaks["bf16_tflops_sustained"], "unit": "TFLOP/s",
                "frac": ach_tf / peaks["bf16_tflops_sustained"], "traffic": traffic,
-               "peak_source": peaks["source"] + " (sustained bf16)", "kernel": "prefix pass",
+               "peak_source": peaks["source"] + " (sustained bf16)", "kernel": wl.attn_kernel,
                "us_per_launch": us_prefix, "alg_flops_per_launch": alg_flops}
     roofline = roof_tc if t_tc_us > t_hbm_us else roof_hbm  # "the slower of" the two bounds
 
@@ -473,7 +477,7 @@ def main():
                               f"inputs larger than L2 ({step_bytes / 2**20:.0f} MiB of distinct KV per step)"),
                        "timing": "CUDA-graph replay of the whole step, CUDA events on the replay stream"},
             "us_per_step": ms_per_step * 1e3,
-            "attn_us_per_layer_prefix_pass": us_prefix,
+            "attn_us_per_layer": us_prefix,
             "roofline": roofline, "roofline_hbm": roof_hbm, "roofline_tensor": roof_tc,
             "gpu_launches": wl.launches_per_step * args.steps,
             "clocks": clocks.summary()}

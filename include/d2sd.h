@@ -99,10 +99,12 @@ int32_t d2sd_build_tree(const int32_t* draft1, const int32_t* draft2, const int3
  * For request b, node t < tree_len[b], head h (kv head g = h / G):
  *   key set = { committed prefix j in [0, ctx_len[b]) }  U  { tree node a : mask[b,t] bit a }
  *   out[b,t,h,:] = softmax_j(sm_scale * q.k_j) . v_j      lse[b,t,h] = ln sum_j exp(sm_scale * q.k_j)
- * computed as: (1) prefix pass -- all T*G query rows of one kv head share one pass over that
- * head's prefix KV, split along the context into `num_splits` chunks (partial (O, LSE) per chunk);
- * (2) tree pass over the <= T_cap tree keys under the ancestor mask; (3) log-sum-exp merge of all
- * partial states.  bf16 in, fp32 accumulate, bf16 out.  Q and tree K are taken post q/k-norm and
+ * computed as a cascade: all T*G query rows of one kv head share one pass over that head's prefix
+ * KV (streamed from HBM once), split along the context into `num_splits` chunks with a partial
+ * (O, LSE) per chunk; the <= T_cap tree keys are attended under the ancestor mask; all partial
+ * states are merged by log-sum-exp.  Contiguous KV with 128 % G == 0 runs as ONE fused tcgen05
+ * launch (tree keys = extra key tiles, merge in the same kernel); other shapes run the mma.sync
+ * kernels (prefix/tree pass + merge).  bf16 in, fp32 accumulate, bf16 out.  Q and tree K are taken post q/k-norm and
  * post-RoPE (pos_id from (b) is for the caller's RoPE).  No sliding window / sinks / soft-cap.
  * ------------------------------------------------------------------------------------------- */
 typedef struct d2sd_attn_params {
@@ -115,16 +117,28 @@ typedef struct d2sd_attn_params {
     int32_t max_ctx_len; /* host-side upper bound on ctx_len[b]; sizes the split-KV grid         */
     int64_t kv_rows;     /* token rows in k_cache/v_cache: contiguous: >= kv_indptr[B] (sum L_b);
                             paged: num_pages * page_size.  Bounds the TMA tensor maps.           */
-    int32_t num_splits;  /* prefix chunks per (request, kv head); 0 = choose from the shape      */
-    int32_t impl;        /* 0 = auto; 1 = force the mma.sync prefix pass; 2 = force tcgen05      */
-    int32_t phases;      /* 0 = all; else bit mask of the phases to enqueue: 1 = prefix pass,
-                            2 = tree pass, 4 = merge.  For profiling and tests: the partial states
-                            stay in the workspace between calls, so 1, 2 and 4 in three calls equal
-                            one call with 0.                                                     */
+    int32_t num_splits;  /* key chunks per (request, kv head); 0 = choose from the shape (<= 64) */
+    int32_t impl;        /* 0 = auto; 1 = force the mma.sync kernels; 2 = force the fused tcgen05
+                            kernel (D2SD_ERR_UNSUPPORTED if the shape is outside it)             */
+    int32_t phases;      /* 0 = the whole cascade.  For tests and profiling: 1 = attend the
+                            committed prefix only, 2 = the tree keys only (out/lse then hold that
+                            state; a prefix-only state with ctx_len = 0 is O = 0, LSE = -inf).
+                            mma.sync kernels only: bit mask of 1 = prefix pass, 2 = tree pass,
+                            4 = merge, the partial states staying in the workspace between calls.*/
 } d2sd_attn_params;
 
-/* Bytes of workspace d2sd_cascade_verify_attn needs for these params (0 on invalid params). */
+/* Bytes of workspace d2sd_cascade_verify_attn needs for these params (0 on invalid params).
+ * Depends on B, T_cap, Hq, Hkv, d, page_size, max_ctx_len, num_splits, impl only. */
 size_t d2sd_cascade_workspace_bytes(const d2sd_attn_params* p /* host */);
+
+/* Prepare a workspace for these params: enqueues a memset of its header (the arrival counters of
+ * the fused kernel) on `stream`.  Call once after allocating the workspace, and again if a kernel of
+ * this library ever failed on it; d2sd_cascade_verify_attn leaves the header zero after every call,
+ * so the same workspace serves any number of calls (and any params it is large enough for) one
+ * after another.  The rest of the workspace is scratch.  Two calls that may run concurrently need
+ * two workspaces. */
+int32_t d2sd_cascade_workspace_init(const d2sd_attn_params* p /* host */, void* workspace,
+                                    size_t workspace_bytes, void* stream);
 
 /*
  *   p           host; read during the call only
@@ -135,7 +149,7 @@ size_t d2sd_cascade_workspace_bytes(const d2sd_attn_params* p /* host */);
  *               paged: offsets into kv_indices
  *   kv_indices  paged: int32 page ids of each request in sequence order; contiguous: NULL
  *   ctx_len     int32 [B], 0 <= ctx_len[b] <= max_ctx_len (0 is legal: the result is the tree state)
- *   tree_k, tree_v    bf16 [B,T_cap,Hkv,d]
+ *   tree_k, tree_v    bf16 [B,T_cap,Hkv,d]; rows t >= tree_len[b] may hold anything (NaN included)
  *   mask        uint32 [B,T_cap,W] as written by d2sd_build_tree (any ancestor-closed mask whose
  *               row n has its self bit and no bit > n is accepted)
  *   tree_len    int32 [B], 1 <= tree_len[b] <= T_cap
@@ -144,7 +158,8 @@ size_t d2sd_cascade_workspace_bytes(const d2sd_attn_params* p /* host */);
  *   dbg_state   NULL, or fp32 [2,B,T_cap,Hq,d+1]: [0] = prefix-only state merged over the chunks,
  *               [1] = tree-only state; each row is the normalised O (d values) followed by its LSE.
  *               For tests: lets the two passes be checked separately.
- *   workspace   >= d2sd_cascade_workspace_bytes(p) bytes, 256-byte aligned; contents are scratch
+ *   workspace   >= d2sd_cascade_workspace_bytes(p) bytes, 256-byte aligned, initialised by
+ *               d2sd_cascade_workspace_init
  * 16-byte alignment is required of q, k_cache, v_cache, tree_k, tree_v and out.
  * Slots of a paged pool that no request owns (including the unused tail of a last page) may hold
  * anything, NaN included: they never reach an output.

@@ -6,5 +6,5 @@ and streams.  There is no CPU fallback: every call raises if the CUDA library is
 """
 from .binding import (  # noqa: F401
     D2sdError, accept, accept_workspace_bytes, build_tree, cascade_verify_attn,
-    cascade_workspace_bytes, last_error, lib, lib_path, select_prefixes, t_cap, version,
+    cascade_workspace, cascade_workspace_bytes, last_error, lib, lib_path, select_prefixes, t_cap, version,
 )

@@ -53,6 +53,8 @@ def lib() -> ctypes.CDLL:
         L.d2sd_build_tree.argtypes = [vp, vp, vp, vp, i32, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp]
         L.d2sd_cascade_workspace_bytes.restype = ctypes.c_size_t
         L.d2sd_cascade_workspace_bytes.argtypes = [ctypes.POINTER(_AttnParams)]
+        L.d2sd_cascade_workspace_init.restype = i32
+        L.d2sd_cascade_workspace_init.argtypes = [ctypes.POINTER(_AttnParams), vp, ctypes.c_size_t, vp]
         L.d2sd_cascade_verify_attn.restype = i32
         L.d2sd_cascade_verify_attn.argtypes = [ctypes.POINTER(_AttnParams)] + [vp] * 14 + [ctypes.c_size_t, vp]
         L.d2sd_accept_workspace_bytes.restype = ctypes.c_size_t
@@ -170,6 +172,19 @@ def cascade_workspace_bytes(B: int, T_cap: int, Hq: int, Hkv: int, d: int, max_c
     return int(n)
 
 
+def cascade_workspace(B: int, T_cap: int, Hq: int, Hkv: int, d: int, max_ctx_len: int, device="cuda",
+                      page_size: int = 0, kv_rows: int = 0, num_splits: int = 0, impl: int = 0) -> torch.Tensor:
+    """Allocate a workspace for these params and initialise it (d2sd_cascade_workspace_init)."""
+    p = _AttnParams(B=B, T_cap=T_cap, Hq=Hq, Hkv=Hkv, d=d, sm_scale=0.0, page_size=page_size,
+                    max_ctx_len=max_ctx_len, kv_rows=kv_rows, num_splits=num_splits, impl=impl, phases=0)
+    n = lib().d2sd_cascade_workspace_bytes(ctypes.byref(p))
+    if n == 0:
+        raise D2sdError(-1, last_error())
+    ws = torch.empty(int(n), dtype=torch.uint8, device=device)
+    _check(lib().d2sd_cascade_workspace_init(ctypes.byref(p), _ptr(ws), int(n), _stream()))
+    return ws
+
+
 def cascade_verify_attn(q: torch.Tensor, k_cache: torch.Tensor, v_cache: torch.Tensor,
                         kv_indptr: Optional[torch.Tensor], kv_indices: Optional[torch.Tensor],
                         ctx_len: torch.Tensor, tree_k: torch.Tensor, tree_v: torch.Tensor, mask: torch.Tensor,
@@ -196,6 +211,7 @@ def cascade_verify_attn(q: torch.Tensor, k_cache: torch.Tensor, v_cache: torch.T
         raise D2sdError(-1, last_error())
     if workspace is None:
         workspace = torch.empty(need, dtype=torch.uint8, device=q.device)
+        _check(lib().d2sd_cascade_workspace_init(ctypes.byref(p), _ptr(workspace), need, _stream()))
     out = _out(out, (B, T_cap, Hq, d), bf, q.device, "out")
     if lse is None and return_lse:
         lse = torch.empty((B, T_cap, Hq), dtype=torch.float32, device=q.device)

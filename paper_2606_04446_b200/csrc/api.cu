@@ -61,7 +61,7 @@ static int32_t make_plan(const d2sd_attn_params* p, AttnPlan* out) {
     pl.kv_rows = p->kv_rows;
     pl.use_tc = false;
     if (p->impl != 1) {
-        pl.use_tc = attn_prefix_tc_supported(pl);
+        pl.use_tc = attn_cascade_tc_supported(pl);
         D2SD_CHECK_SUPPORTED(pl.use_tc || p->impl != 2, "impl = 2 (tcgen05) does not cover this shape");
     }
     const int rows = pl.T_cap * pl.G;
@@ -69,29 +69,29 @@ static int32_t make_plan(const d2sd_attn_params* p, AttnPlan* out) {
     int splits = p->num_splits;
     if (pl.use_tc) {
         // One wave of CTA pairs (1 CTA/SM): a work item (request, kv head, group of <= 3 query tiles,
-        // chunk) is served by two CTAs.  Chunks are multiples of 16 keys (the MMA N granularity).
+        // chunk of key tiles) is served by two CTAs.  The key tiles of a request are its prefix tiles
+        // followed by its tree tiles; the kernel cuts them into num_splits chunks of whole tiles.
         pl.n_mgroups = ceil_div(rows, 384);
         pl.rows_pad = pl.n_mgroups * 384;
+        const int max_tiles = ceil_div(p->max_ctx_len, 128) + ceil_div(pl.T_cap, 128);
         if (splits == 0) {
             const int64_t per_split = (int64_t)pl.B * pl.Hkv * pl.n_mgroups;
             splits = (int)((sm_count() / 2) / (per_split > 0 ? per_split : 1));
-            if (splits < 1) splits = 1;
-            const int max_splits = (max_ctx + 127) / 128;  // never below one 128-key tile per chunk
-            if (splits > max_splits) splits = max_splits;
             if (splits > 64) splits = 64;
         }
-        D2SD_CHECK_SUPPORTED(splits <= 16384, "num_splits = %d too large", splits);
-        pl.chunk_keys = (ceil_div(max_ctx, splits) + 15) / 16 * 16;
-        pl.num_splits = ceil_div(max_ctx, pl.chunk_keys);
+        if (splits > 64) splits = 64;                // a group's 2*splits CTAs wait for each other: one wave
+        if (splits > max_tiles) splits = max_tiles;  // never an always-empty chunk
+        if (splits < 1) splits = 1;
+        pl.chunk_keys = 0;
+        pl.num_splits = splits;
         pl.NSLOT = 2 * pl.num_splits;
-        pl.NS = 1;  // the tree state, row layout
+        pl.NS = 0;
         const size_t slot_rows = (size_t)pl.B * pl.NSLOT * pl.Hkv * pl.rows_pad;
-        const size_t tree_rows = (size_t)pl.B * pl.T_cap * pl.Hq;
-        pl.off_o = 0;
-        pl.off_lse = align_up(slot_rows * pl.d * sizeof(float), 256);
-        pl.off_tree_o = pl.off_lse + align_up(slot_rows * sizeof(float), 256);
-        pl.off_tree_lse = pl.off_tree_o + align_up(tree_rows * pl.d * sizeof(float), 256);
-        pl.bytes = pl.off_tree_lse + align_up(tree_rows * sizeof(float), 256);
+        pl.off_cnt = 0;
+        pl.cnt_bytes = align_up((size_t)pl.B * pl.Hkv * pl.n_mgroups * 2 * sizeof(unsigned), 256);
+        pl.off_o = pl.cnt_bytes;
+        pl.off_lse = pl.off_o + align_up(slot_rows * pl.d * sizeof(float), 256);
+        pl.bytes = pl.off_lse + align_up(slot_rows * sizeof(float), 256);
     } else {
         if (splits == 0) {
             // ~3 CTAs/SM of 64-row M blocks
@@ -107,6 +107,8 @@ static int32_t make_plan(const d2sd_attn_params* p, AttnPlan* out) {
         pl.num_splits = ceil_div(max_ctx, pl.chunk_keys);
         pl.NS = pl.num_splits + 1;
         const size_t rows_all = (size_t)pl.B * pl.NS * pl.T_cap * pl.Hq;
+        pl.off_cnt = 0;
+        pl.cnt_bytes = 0;
         pl.off_o = 0;
         pl.off_lse = align_up(rows_all * pl.d * sizeof(float), 256);
         pl.bytes = pl.off_lse + align_up(rows_all * sizeof(float), 256);
@@ -195,25 +197,35 @@ int32_t d2sd_cascade_verify_attn(const d2sd_attn_params* p, const void* q, const
     const int phases = p->phases ? p->phases : 7;
     const bool do_prefix = phases & 1, do_tree = phases & 2, do_merge = phases & 4;
     if (pl.use_tc) {
-        a.tree_o = reinterpret_cast<float*>(static_cast<char*>(workspace) + pl.off_tree_o);
-        a.tree_lse = reinterpret_cast<float*>(static_cast<char*>(workspace) + pl.off_tree_lse);
-        if (do_prefix)
-            if (int32_t st = launch_attn_prefix_tc(pl, a, s)) return st;
-        if (do_tree) {  // the tree state goes to its own row-layout region: a plan with no prefix chunks
-            AttnPlan tp = pl;
-            tp.num_splits = 0;
-            tp.NS = 1;
-            AttnArgs ta = a;
-            ta.part_o = a.tree_o;
-            ta.part_lse = a.tree_lse;
-            if (int32_t st = launch_attn_mma(tp, ta, /*prefix=*/false, /*tree=*/true, s)) return st;
+        // One fused launch: prefix tiles, tree tiles and the cascade merge.  phases selects which key
+        // tiles take part (1 = prefix only, 2 = tree only); dbg_state costs two extra launches.
+        a.counters = reinterpret_cast<unsigned*>(static_cast<char*>(workspace) + pl.off_cnt);
+        if (dbg_state) {
+            const size_t half = (size_t)pl.B * pl.T_cap * pl.Hq * (pl.d + 1);
+            if (int32_t st = launch_attn_cascade_tc(pl, a, 1, dbg_state, s)) return st;
+            if (int32_t st = launch_attn_cascade_tc(pl, a, 2, dbg_state + half, s)) return st;
         }
-        if (do_merge) return launch_attn_merge_tc(pl, a, s);
-        return D2SD_OK;
+        const int mode = phases & 3;
+        if (mode == 0) return D2SD_OK;  // phases == 4: the merge is part of the launch
+        return launch_attn_cascade_tc(pl, a, mode, nullptr, s);
     }
     if (do_prefix || do_tree)
         if (int32_t st = launch_attn_mma(pl, a, do_prefix, do_tree, s)) return st;
     if (do_merge) return launch_attn_merge(pl, a, s);
+    return D2SD_OK;
+}
+
+int32_t d2sd_cascade_workspace_init(const d2sd_attn_params* p, void* workspace, size_t workspace_bytes,
+                                    void* stream) {
+    clear_error();
+    AttnPlan pl;
+    if (int32_t st = make_plan(p, &pl)) return st;
+    if (workspace == nullptr || workspace_bytes < pl.bytes || (reinterpret_cast<uintptr_t>(workspace) & 255))
+        return set_error(D2SD_ERR_WORKSPACE, "workspace %p with %zu bytes; need %zu bytes, 256-byte aligned",
+                         workspace, workspace_bytes, pl.bytes);
+    if (pl.cnt_bytes)
+        D2SD_CHECK_CUDA(cudaMemsetAsync(static_cast<char*>(workspace) + pl.off_cnt, 0, pl.cnt_bytes,
+                                        static_cast<cudaStream_t>(stream)));
     return D2SD_OK;
 }
 

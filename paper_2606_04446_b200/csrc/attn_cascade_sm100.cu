@@ -1,9 +1,13 @@
-// Stage (c) prefix pass on tcgen05 / TMEM / TMA (sm_100a).  PAPER.md:52, :124, :154.
+// Stage (c), fused: cascade tree-verify attention in ONE launch on tcgen05 / TMEM / TMA (sm_100a).
+// PAPER.md:52, :124, :154.
 //
 // Every tree query of every branch and every GQA head of one kv head is a row of one batched query
 // matrix (row r = t*G + hh), cut into 128-row M tiles; up to three M tiles form an "M group".  The
-// context is cut into `num_splits` chunks.  One work item = (request b, kv head g, M group, chunk)
-// and is served by a PAIR of CTAs (rank 0 / 1) that stream the same K/V chunk:
+// keys of a request are the committed prefix followed by the tree-local keys, cut into 128-key
+// tiles: prefix tiles 0..np-1 (np = ceil(L/128)) and tree tiles np..np+nt-1 (nt = ceil(T/128)); the
+// tree tiles are ordinary key tiles whose scores additionally pass the node's ancestor-mask bits.
+// The tile sequence is cut into `num_splits` chunks.  One work item = (request b, kv head g, M
+// group, chunk) and is served by a PAIR of CTAs (rank 0 / 1) that stream the same K/V chunk:
 //
 //   M tiles in the group   rank 0 computes                rank 1 computes
 //   3                      tile 0 (all key tiles)         tile 1 (all key tiles)
@@ -23,16 +27,26 @@
 // instruction against 64 ideal; N = 64 instructions are issue/SMEM-bound at 54 cycles against 32).
 //
 // Warp roles (384 threads): warp 0 = TMA producer, warp 1 = MMA issuer (one thread), warp 2 = TMEM
-// allocator, warps 4..11 = softmax: two threads per query row (TMEM lane), warps 4..7 on key columns
-// 0..63 and warps 8..11 on columns 64..127 of every S tile, so that two warps per scheduler share
-// the MUFU pipe; the halves exchange row maxima through shared memory.  Running max / sum stay in
-// registers; the running max is only raised when a tile maximum exceeds it by more than 2^8 (lazy
-// rescale), in which case the owning threads rescale their O row in TMEM before the next P.V.
+// allocator, warp 3 = zeroes the V rows behind a ragged tile end (they are multiplied by exact zeros
+// and may hold anything, NaN included), warps 4..11 = softmax: two threads per query row (TMEM
+// lane), warps 4..7 on key columns 0..63 and warps 8..11 on columns 64..127 of every S tile, so that
+// two warps per scheduler share the MUFU pipe; the halves exchange row maxima through shared
+// memory.  Running max / sum stay in registers; the running max is only raised when a tile maximum
+// exceeds it by more than 2^8 (lazy rescale), in which case the owning threads rescale their O row
+// in TMEM before the next P.V.
 //
-// Output: one partial state (normalised O fp32, LSE) per (chunk, rank) "slot", transposed through
-// shared memory (XOR-swizzled 16-byte chunks, conflict-free) and written as whole 512-byte rows.
-// Workspace layout (private to this file and the merge kernel below): O [b][slot][g][rows_pad][128]
-// fp32, LSE [b][slot][g][rows_pad].
+// Cascade merge in the same launch (log-sum-exp state merge): every CTA writes one
+// partial state (normalised O fp32, LSE) per accumulator slot to the workspace (it stays in L2),
+// publishes it with a release-increment of its group's arrival counter, waits until all
+// 2*num_splits CTAs of the group (same b, g, M group) have arrived, and then merges ITS share of the
+// group's rows (rows are dealt round-robin to the group's softmax warps) and writes the bf16 output
+// and the LSE.  The counters reset themselves (last CTA out), so the workspace header only has to
+// be zero before the first call (d2sd_cascade_workspace_init).  The wait is safe because a group is
+// 2*num_splits consecutive blocks of the grid's linear order: the oldest unfinished group always
+// has all its CTAs resident or done; the spin is bounded and traps instead of hanging.
+// Workspace layout (private to this file): header of arrival/done counters, then O
+// [b][slot][g][rows_pad][128] fp32 (XOR-swizzled 16-byte chunks are undone before the store) and
+// LSE [b][slot][g][rows_pad].
 #include <cuda.h>
 
 #include "common.cuh"
@@ -70,7 +84,9 @@ enum : uint32_t {
     kBarPFull = kBarSFull + 2,         // [2]
     kBarODone = kBarPFull + 2,         // [2]
     kBarAllDone = kBarODone + 2,       // every MMA of the CTA has completed
-    kNumBars = kBarAllDone + 1,
+    kBarVFix = kBarAllDone + 1,        // [2] warp 3 has zeroed the V rows behind a ragged tile end; a CTA
+                                       // meets at most two ragged tiles (last prefix tile, last tree tile)
+    kNumBars = kBarVFix + 2,
     kTmemSlot = kNumBars  // uint32 written by tcgen05.alloc
 };
 static_assert((kNumBars + 1) * 8 <= 256, "barrier area");
@@ -127,15 +143,6 @@ __device__ __forceinline__ void tma_load_5d(uint32_t dst, const CUtensorMap* tm,
 }
 __device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* tm) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(tm)) : "memory");
-}
-// shared -> global bulk copy (no tensor map: the destination is one contiguous run of rows)
-__device__ __forceinline__ void bulk_store(void* gdst, uint32_t ssrc, uint32_t bytes) {
-    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(ssrc), "r"(bytes)
-                 : "memory");
-}
-__device__ __forceinline__ void bulk_commit_wait_read() {
-    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
 }
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void named_bar_sync(uint32_t id, uint32_t threads) {
@@ -245,9 +252,83 @@ __device__ long long g_timeline[256][128];
 #endif
 
 // -------------------------------------------------------------------------------------------------
+// Cascade merge of one group's rows (log-sum-exp state merge):
+//   LSE = log sum_p e^{LSE_p};  O = sum_p e^{LSE_p - LSE} O_p   over the slots that hold the row's M tile.
+// Warp `gw` of `n_gw` takes rows gw, gw + n_gw, ... of the group; lane i first fetches the LSE of
+// relevant slot i, then the warp sweeps the slots' O rows (512 B each, coalesced).  The partial
+// states were written by other SMs: read them at L2 (ld.global.cg).
+__device__ __forceinline__ void merge_rows(const AttnPlan& pl, const AttnArgs& a, float* dbg_rows, int b, int g,
+                                           int row_base, int rows_g, int MT, int gw, int n_gw, int lane) {
+    const int G = pl.G;
+    for (int rr = gw; rr < rows_g; rr += n_gw) {
+        const int r = row_base + rr;
+        const int tl = rr / kTileM;
+        const bool own = MT >= 2 && tl < 2;  // tile owned by rank tl; otherwise shared by both ranks
+        const int n_rel = own ? pl.num_splits : 2 * pl.num_splits;  // relevant slots
+        auto row_of = [&](int i) {
+            const int slot = own ? 2 * i + tl : i;
+            return (((size_t)b * pl.NSLOT + slot) * pl.Hkv + g) * pl.rows_pad + r;
+        };
+        float m = -INFINITY, wsum = 0.f;
+        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int base = 0; base < n_rel; base += 32) {
+            const int i = base + lane;
+            const float l = i < n_rel ? __ldcg(a.part_lse + row_of(i)) : -INFINITY;
+            float mb = l;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) mb = fmaxf(mb, __shfl_xor_sync(0xffffffffu, mb, o));
+            if (mb == -INFINITY) continue;
+            if (mb > m) {  // rescale what has been accumulated so far (only with > 32 relevant slots)
+                const float sc = m == -INFINITY ? 0.f : __expf(m - mb);
+                acc.x *= sc; acc.y *= sc; acc.z *= sc; acc.w *= sc;
+                wsum *= sc;
+                m = mb;
+            }
+            const float wl = l == -INFINITY ? 0.f : __expf(l - m);
+            const int cnt = min(32, n_rel - base);
+#pragma unroll 6
+            for (int q = 0; q < cnt; ++q) {
+                const float w = __shfl_sync(0xffffffffu, wl, q);
+                if (w == 0.f) continue;
+                const float4 o = __ldcg(reinterpret_cast<const float4*>(a.part_o + row_of(base + q) * kD) + lane);
+                wsum += w;
+                acc.x += w * o.x; acc.y += w * o.y; acc.z += w * o.z; acc.w += w * o.w;
+            }
+        }
+        const float inv = wsum > 0.f ? 1.f / wsum : 0.f;  // no key at all (L = 0, prefix-only mode): O = 0, LSE = -inf
+        const float lse = wsum > 0.f ? m + logf(wsum) : -INFINITY;
+        const int t = r / G;
+        const size_t orow = ((size_t)b * pl.T_cap + t) * pl.Hq + g * G + (r - t * G);
+        if (dbg_rows) {  // fp32 state for tests: d values of O, then the LSE
+            float* d0 = dbg_rows + orow * (kD + 1);
+            d0[lane * 4 + 0] = acc.x * inv; d0[lane * 4 + 1] = acc.y * inv;
+            d0[lane * 4 + 2] = acc.z * inv; d0[lane * 4 + 3] = acc.w * inv;
+            if (lane == 0) d0[kD] = lse;
+            continue;
+        }
+        __nv_bfloat162 lo = __floats2bfloat162_rn(acc.x * inv, acc.y * inv);
+        __nv_bfloat162 hi = __floats2bfloat162_rn(acc.z * inv, acc.w * inv);
+        uint2 pk;
+        pk.x = *reinterpret_cast<uint32_t*>(&lo);
+        pk.y = *reinterpret_cast<uint32_t*>(&hi);
+        *reinterpret_cast<uint2*>(a.out + orow * kD + lane * 4) = pk;
+        if (a.lse && lane == 0) a.lse[orow] = lse;
+    }
+}
+
+// mode bits: 1 = include the prefix tiles, 2 = include the tree tiles (3 = the whole cascade).
+struct TileInfo {
+    int valid;      // keys of the tile that exist (1..128)
+    int row;        // first row of the tile in its tensor map
+    bool tree;      // tree tile (ancestor mask applies), else prefix tile
+    int tt;         // tree tile index (tree tiles only)
+};
+
 __global__ void __launch_bounds__(kThreads, 1)
-attn_prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
-                      const __grid_constant__ CUtensorMap tm_v, AttnPlan pl, AttnArgs a) {
+attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
+                       const __grid_constant__ CUtensorMap tm_v, const __grid_constant__ CUtensorMap tm_tk,
+                       const __grid_constant__ CUtensorMap tm_tv, AttnPlan pl, AttnArgs a, int mode,
+                       float* dbg_rows) {
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     const uint32_t smem_raw_u32 = (uint32_t)__cvta_generic_to_shared(smem_raw);
     const uint32_t smem = (smem_raw_u32 + 1023u) & ~1023u;  // 128B swizzle atoms need 1024 B alignment
@@ -260,30 +341,34 @@ attn_prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
     const int rank = blockIdx.x & 1, split = blockIdx.x >> 1, g = blockIdx.y;
     const int b = blockIdx.z / pl.n_mgroups, mg = blockIdx.z - b * pl.n_mgroups;
     const int G = pl.G;
-    const int rows_valid = a.tree_len[b] * G;
+    const int T = a.tree_len[b];
+    const int rows_valid = T * G;
     const int row_base = mg * (kGroupTiles * kTileM);
-    if (row_base >= rows_valid) return;
-    const int MT = min(kGroupTiles, (rows_valid - row_base + kTileM - 1) / kTileM);
+    if (row_base >= rows_valid) return;  // the whole group returns: nobody waits for it
+    const int rows_g = min(kGroupTiles * kTileM, rows_valid - row_base);
+    const int MT = (rows_g + kTileM - 1) / kTileM;
     const SlotPlan sp = make_slots(MT, rank);
     const int L = a.ctx_len[b];
-    const int k_begin = split * pl.chunk_keys;
-    const int k_end = min(L, k_begin + pl.chunk_keys);
+    // key tiles of this request: prefix tiles [0, np), tree tiles [np, np + nt); this chunk: [j_begin, j_end)
+    const int np = (mode & 1) ? (L + kTileN - 1) / kTileN : 0;
+    const int nt = (mode & 2) ? (T + kTileN - 1) / kTileN : 0;
+    const int tps = max(1, (np + nt + pl.num_splits - 1) / pl.num_splits);
+    const int j_begin = split * tps;
+    const int n_tiles = max(0, min(np + nt, j_begin + tps) - j_begin);
     const int slot_id = 2 * split + rank;
     const size_t slot_row0 = (((size_t)b * pl.NSLOT + slot_id) * pl.Hkv + g) * pl.rows_pad;
     float* po = a.part_o + slot_row0 * kD;
     float* plse = a.part_lse + slot_row0;
-    const int n_tiles = k_begin < k_end ? (k_end - k_begin + kTileN - 1) / kTileN : 0;
-    if (n_tiles == 0) {  // empty chunk: state (O = 0, LSE = -inf); O is never read by the merge
-        for (int s = 0; s < 2; ++s) {
-            if (sp.tile[s] < 0) continue;
-            const int r0 = row_base + sp.tile[s] * kTileM;
-            for (int r = r0 + tid; r < min(rows_valid, r0 + kTileM); r += kThreads) plse[r] = -INFINITY;
-        }
-        return;
-    }
-    const int kv_row0 = (a.kv_indptr ? a.kv_indptr[b] : 0) + k_begin;
-    const int last_valid = (k_end - k_begin) - (n_tiles - 1) * kTileN;  // valid keys of the last key tile
-    const int last_n = (last_valid + 15) & ~15;                         // its MMA N (multiple of 16)
+    const int kv_row0 = a.kv_indptr ? a.kv_indptr[b] : 0;
+    auto tile_info = [&](int jj) {
+        const int j = j_begin + jj;
+        TileInfo ti;
+        ti.tree = j >= np;
+        ti.tt = j - np;
+        ti.valid = ti.tree ? min(kTileN, T - ti.tt * kTileN) : min(kTileN, L - j * kTileN);
+        ti.row = ti.tree ? b * pl.T_cap + ti.tt * kTileN : kv_row0 + j * kTileN;
+        return ti;
+    };
 
     const uint32_t bar0 = smem + kOffBar;
     auto bar = [&](uint32_t i) { return bar0 + 8u * i; };
@@ -294,7 +379,7 @@ attn_prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
         mbar_init(bar(kBarQFull + 1), 1);
         for (int i = 0; i < kRing; ++i) {
             mbar_init(bar(kBarFull + i), 1);
-            mbar_init(bar(kBarEmpty + i), 1);
+            mbar_init(bar(kBarEmpty + i), 2);  // the MMA's commit + the V sanitiser
         }
         for (int s = 0; s < 2; ++s) {
             mbar_init(bar(kBarSFull + s), 1);
@@ -302,10 +387,14 @@ attn_prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
             mbar_init(bar(kBarODone + s), 1);
         }
         mbar_init(bar(kBarAllDone), 1);
+        mbar_init(bar(kBarVFix + 0), 1);
+        mbar_init(bar(kBarVFix + 1), 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         tma_prefetch_desc(&tm_q);
         tma_prefetch_desc(&tm_k);
         tma_prefetch_desc(&tm_v);
+        tma_prefetch_desc(&tm_tk);
+        tma_prefetch_desc(&tm_tv);
     }
     if (warp == 2) {
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(bar(kTmemSlot)),
@@ -326,12 +415,14 @@ attn_prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
             bool q_sent = false;
             for (int j = 0; j < n_tiles; ++j) {
                 if (!sp.used(j, rank)) continue;
+                const TileInfo ti = tile_info(j);
                 for (int kv = 0; kv < 2; ++kv, ++x) {
                     const int i = x % kRing;
                     mbar_wait(bar(kBarEmpty + i), ((x / kRing) & 1) ^ 1);
                     mbar_expect_tx(bar(kBarFull + i), kKvTileBytes);
-                    tma_load_4d(smem + kOffRing + i * kKvTileBytes, kv ? &tm_v : &tm_k, bar(kBarFull + i), 0,
-                                kv_row0 + j * kTileN, 0, g, kEvictFirst);
+                    const CUtensorMap* tm = ti.tree ? (kv ? &tm_tv : &tm_tk) : (kv ? &tm_v : &tm_k);
+                    tma_load_4d(smem + kOffRing + i * kKvTileBytes, tm, bar(kBarFull + i), 0, ti.row, 0, g,
+                                ti.tree ? kEvictLast : kEvictFirst);
                     if (!q_sent) {
                         q_sent = true;
                         for (int s = 0; s < 2; ++s) {
@@ -355,12 +446,14 @@ attn_prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
             // the PV that is still owed (unit n-1)
             bool pend = false, pend_last = false;
             int pend_slot = 0, pend_sbuf = 0, pend_vx = 0, pend_n = 0;
-            bool v_waited = false;
+            bool v_waited = false, pend_ragged = false;
+            int n_ragged = 0;
             auto do_pv = [&]() {
                 const int s = pend_slot, vi = pend_vx % kRing;
                 mbar_wait(bar(kBarPFull + s), cnt_pv[s] & 1);
                 if (!v_waited) {
                     mbar_wait(bar(kBarFull + vi), (pend_vx / kRing) & 1);
+                    if (pend_ragged) mbar_wait(bar(kBarVFix + n_ragged++), 0);
                     v_waited = true;
                 }
                 tc_fence_after();
@@ -381,7 +474,8 @@ attn_prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
                 const int kx = x, vx = x + 1;
                 x += 2;
                 const int ki = kx % kRing;
-                const int tile_n = (j == n_tiles - 1) ? last_n : kTileN;
+                const int valid = tile_info(j).valid;
+                const int tile_n = (valid + 15) & ~15;  // MMA N of Q.K^T and K extent of P.V (multiple of 16)
                 const bool sh = sp.shared_on(j, rank);
                 mbar_wait(bar(kBarFull + ki), (kx / kRing) & 1);
                 const uint64_t kd = smem_desc(smem + kOffRing + ki * kKvTileBytes, 16, 1024);
@@ -407,12 +501,45 @@ attn_prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
                     }
                     pend = true; pend_slot = s; pend_sbuf = n & 1; pend_vx = vx; pend_n = tile_n;
                     pend_last = last_of_tile;
+                    pend_ragged = (valid & 15) != 0;
                     if (s == 0 || !sp.own()) v_waited = false;  // first unit of this key tile: V_j not yet waited for
                     ++n;
                 }
             }
             if (pend) do_pv();
             tc_commit(bar(kBarAllDone));
+        }
+    } else if (warp == 3) {
+        // ===== V sanitiser: the P.V MMA runs over ceil16(valid) keys; rows valid..ceil16(valid)-1 of a
+        // ragged V tile belong to nobody (next request, tree padding) and are multiplied by P = 0
+        // exactly, so they must not hold NaN/Inf: zero them in shared memory.  A row is 2 x 128 B
+        // (d halves); the 128B swizzle permutes 16-byte chunks inside a row's 128 B only.
+        // The warp observes EVERY fill of every ring slot in order (a parity wait is only sound
+        // then) and is the second arriver on each slot's empty barrier, so it can never be lapped. =====
+        int x = 0, n_ragged = 0;
+        for (int j = 0; j < n_tiles; ++j) {
+            if (!sp.used(j, rank)) continue;
+            const int valid = tile_info(j).valid;
+            for (int kv = 0; kv < 2; ++kv, ++x) {
+                const int i = x % kRing;
+                mbar_wait(bar(kBarFull + i), (x / kRing) & 1);
+                if (kv == 1 && (valid & 15) != 0) {
+                    const int n_rows = ((valid + 15) & ~15) - valid;
+                    for (int e = lane; e < n_rows * 16; e += 32) {  // 16 x 16 B per row
+                        const int row = valid + (e >> 4), c16 = e & 15;
+                        const uint32_t addr = smem + kOffRing + i * kKvTileBytes +
+                                              (uint32_t)(c16 >> 3) * (kKvTileBytes / 2) + (uint32_t)row * 128u +
+                                              (uint32_t)(c16 & 7) * 16u;
+                        asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(addr), "r"(0u) : "memory");
+                    }
+                    fence_async_smem();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(bar(kBarVFix + n_ragged));
+                    ++n_ragged;
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar(kBarEmpty + i));
+            }
         }
     } else if (warp >= 4) {
         // ===== softmax: warps 4..7 take key columns 0..63 of every S tile, warps 8..11 columns 64..127;
@@ -431,7 +558,8 @@ attn_prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
         for (int j = 0; j < n_tiles; ++j) {
             if (!sp.used(j, rank)) continue;
             const bool sh = sp.shared_on(j, rank);
-            const bool last_tile = (j == n_tiles - 1) && last_valid < kTileN;
+            const TileInfo ti = tile_info(j);
+            const bool masked_tile = ti.tree || ti.valid < kTileN;
 #pragma unroll
             for (int s = 0; s < 2; ++s) {
                 if (s == 0 ? !sp.own() : !sh) continue;
@@ -448,10 +576,23 @@ attn_prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
                     D2SD_TMEM_LD32(sbuf + h * 64, sv, 0);
                     D2SD_TMEM_LD32(sbuf + h * 64 + 32, sv, 32);
                     tmem_wait_ld();
-                    if (last_tile) {
+                    if (masked_tile) {
+                        // keys past the tile's end, and (tree tiles) keys that are not ancestors-or-self of
+                        // this row's node: bits 64h..64h+63 of the tile's 128 mask bits, -> -inf
+                        uint32_t mw0 = 0xFFFFFFFFu, mw1 = 0xFFFFFFFFu;
+                        if (ti.tree) {
+                            const int t = min((row_base + sp.tile[s] * kTileM + rl) / G, T - 1);
+                            const uint32_t* mrow = a.mask + ((size_t)b * pl.T_cap + t) * pl.W;
+                            const int wi = ti.tt * 4 + h * 2;
+                            mw0 = wi < pl.W ? mrow[wi] : 0u;
+                            mw1 = wi + 1 < pl.W ? mrow[wi + 1] : 0u;
+                        }
+                        const int lim = ti.valid - h * 64;  // columns [lim, 64) of this half are past the end
 #pragma unroll
-                        for (int c = 0; c < 64; ++c)
-                            if (h * 64 + c >= last_valid) sv[c] = 0xFF800000u;  // -inf: keys outside the chunk
+                        for (int c = 0; c < 64; ++c) {
+                            const uint32_t bit = ((c < 32 ? mw0 : mw1) >> (c & 31)) & 1u;
+                            if (c >= lim || !bit) sv[c] = 0xFF800000u;
+                        }
                     }
                     float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;
 #pragma unroll
@@ -492,7 +633,8 @@ attn_prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
                             l_run[s] *= alpha;
                         }
                     }
-                    const float ms = m_run[s] * c2;
+                    // a row with every key so far masked has m_run = -inf: exp2(-inf - 0) = 0, not NaN
+                    const float ms = m_run[s] == -INFINITY ? 0.f : m_run[s] * c2;
                     float sum0 = 0.f, sum1 = 0.f;
                     uint32_t p[32];
 #pragma unroll
@@ -539,7 +681,7 @@ attn_prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
             const uint32_t stage = smem + kOffRing + (uint32_t)s * (2 * kKvTileBytes);
             if (warp_active) {
                 tc_fence_after();
-                const float inv = 1.f / l_tot;
+                const float inv = l_tot > 0.f ? 1.f / l_tot : 0.f;  // l = 0: every key of the chunk masked
                 const uint32_t srow = stage + (uint32_t)rl * 512u;
                 const uint32_t o_addr = tmem + s * kD + h * 64 + lane_addr;
 #pragma unroll
@@ -557,7 +699,7 @@ attn_prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
                                      : "memory");
                     }
                 }
-                if (h == 0 && row_ok) plse[r] = m_run[s] * pl.sm_scale + logf(l_tot);
+                if (h == 0 && row_ok) plse[r] = l_tot > 0.f ? m_run[s] * pl.sm_scale + logf(l_tot) : -INFINITY;
             }
             named_bar_sync(1, 256);
             // warp q of the eight stores rows q*16 .. q*16+15, one 512-byte row per instruction
@@ -578,6 +720,35 @@ attn_prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
             }
         }
         if (warp == 4 && lane == 0) TL(101);
+
+        // ---- publish this CTA's partial states, wait for the group, merge this CTA's share of rows ----
+        const unsigned expected = gridDim.x;  // 2 * num_splits CTAs per (b, g, M group)
+        unsigned* cnt = a.counters + 2 * (blockIdx.z * gridDim.y + blockIdx.y);  // [0] arrivals, [1] done
+        __threadfence();
+        named_bar_sync(1, 256);
+        if (warp == 4 && lane == 0) {
+            asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(cnt) : "memory");
+            unsigned seen, spins = 0;
+            do {
+                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(cnt) : "memory");
+                if (seen < expected) {
+                    __nanosleep(32);
+                    if (++spins > (1u << 24)) __trap();  // a scheduling assumption broke: fail, do not hang
+                }
+            } while (seen < expected);
+        }
+        named_bar_sync(1, 256);
+        if (warp == 4 && lane == 0) TL(102);
+        merge_rows(pl, a, dbg_rows, b, g, row_base, rows_g, MT, (int)blockIdx.x * 8 + (warp - 4), (int)gridDim.x * 8,
+                   lane);
+        named_bar_sync(1, 256);
+        if (warp == 4 && lane == 0) {
+            if (atomicAdd(cnt + 1, 1u) == expected - 1) {  // last CTA out: everybody is past the wait
+                cnt[0] = 0;
+                cnt[1] = 0;
+            }
+            TL(103);
+        }
     }
 
     tc_fence_before();
@@ -586,84 +757,6 @@ attn_prefix_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_con
     if (warp == 2) {
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(kTmemCols) : "memory");
     }
-}
-
-// Merge for the tcgen05 path: LSE = log sum_p e^{LSE_p};  O = sum_p e^{LSE_p - LSE} O_p over the slots
-// that hold the row's M tile and the tree state ("cascade attention" state merge).
-// One warp per (b,t,h) row; lane i first fetches the LSE of relevant slot i, then the warp sweeps
-// the slots' O rows (512 B each, coalesced).
-__global__ void __launch_bounds__(128) attn_merge_tc_kernel(AttnPlan pl, AttnArgs a) {
-    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
-    const int rows_per_req = pl.T_cap * pl.Hq;
-    if (warp >= pl.B * rows_per_req) return;
-    const int b = warp / rows_per_req;
-    const int th = warp - b * rows_per_req;  // t*Hq + h
-    const int t = th / pl.Hq, h = th - t * pl.Hq;
-    const int T = a.tree_len[b];
-    if (t >= T) return;
-    const int G = pl.G, g = h / G;
-    const int r = t * G + (h - g * G);
-    const int mg = r / (kGroupTiles * kTileM);
-    const int tl = (r - mg * kGroupTiles * kTileM) / kTileM;
-    const int MT = min(kGroupTiles, (T * G - mg * kGroupTiles * kTileM + kTileM - 1) / kTileM);
-    const bool own = MT >= 2 && tl < 2;       // tile owned by rank tl; otherwise shared by both ranks
-    const int n_rel = own ? pl.num_splits : 2 * pl.num_splits;  // relevant slots (<= 128)
-    auto slot_of = [&](int i) { return own ? 2 * i + tl : i; };
-    auto row_of = [&](int slot) { return (((size_t)b * pl.NSLOT + slot) * pl.Hkv + g) * pl.rows_pad + r; };
-
-    float m = -INFINITY, wsum = 0.f;
-    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-    for (int base = 0; base < n_rel; base += 32) {
-        const int i = base + lane;
-        const float l = i < n_rel ? a.part_lse[row_of(slot_of(i))] : -INFINITY;
-        float mb = l;
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) mb = fmaxf(mb, __shfl_xor_sync(0xffffffffu, mb, o));
-        if (mb == -INFINITY) continue;
-        if (mb > m) {  // rescale what has been accumulated so far (only with > 32 relevant slots)
-            const float sc = m == -INFINITY ? 0.f : __expf(m - mb);
-            acc.x *= sc; acc.y *= sc; acc.z *= sc; acc.w *= sc;
-            wsum *= sc;
-            m = mb;
-        }
-        const float wl = l == -INFINITY ? 0.f : __expf(l - m);
-        const int cnt = min(32, n_rel - base);
-#pragma unroll 4
-        for (int q = 0; q < cnt; ++q) {
-            const float w = __shfl_sync(0xffffffffu, wl, q);
-            if (w == 0.f) continue;
-            const float4 o = *reinterpret_cast<const float4*>(a.part_o + row_of(slot_of(base + q)) * kD + lane * 4);
-            wsum += w;
-            acc.x += w * o.x; acc.y += w * o.y; acc.z += w * o.z; acc.w += w * o.w;
-        }
-    }
-    const float lse_prefix = (m > -INFINITY) ? m + logf(wsum) : -INFINITY;
-    const float lt = a.tree_lse[(size_t)b * rows_per_req + th];
-    const float4 ot = *reinterpret_cast<const float4*>(a.tree_o + ((size_t)b * rows_per_req + th) * kD + lane * 4);
-    if (a.dbg_state) {
-        const size_t rs = (size_t)(kD + 1);
-        float* d0 = a.dbg_state + ((size_t)b * rows_per_req + th) * rs;
-        float* d1 = d0 + (size_t)pl.B * rows_per_req * rs;
-        const float inv = wsum > 0.f ? 1.f / wsum : 0.f;
-        d0[lane * 4 + 0] = acc.x * inv; d0[lane * 4 + 1] = acc.y * inv;
-        d0[lane * 4 + 2] = acc.z * inv; d0[lane * 4 + 3] = acc.w * inv;
-        d1[lane * 4 + 0] = ot.x; d1[lane * 4 + 1] = ot.y; d1[lane * 4 + 2] = ot.z; d1[lane * 4 + 3] = ot.w;
-        if (lane == 0) { d0[kD] = lse_prefix; d1[kD] = lt; }
-    }
-    // fold the tree state in (lt is finite: every row has its self bit)
-    const float m2 = fmaxf(m, lt);
-    const float sp = (m > -INFINITY) ? __expf(m - m2) : 0.f;
-    const float wt = __expf(lt - m2);
-    const float tot = wsum * sp + wt;
-    const float inv = 1.f / tot;
-    const float ox = (acc.x * sp + wt * ot.x) * inv, oy = (acc.y * sp + wt * ot.y) * inv;
-    const float oz = (acc.z * sp + wt * ot.z) * inv, ow = (acc.w * sp + wt * ot.w) * inv;
-    __nv_bfloat162 lo = __floats2bfloat162_rn(ox, oy), hi = __floats2bfloat162_rn(oz, ow);
-    uint2 pk;
-    pk.x = *reinterpret_cast<uint32_t*>(&lo);
-    pk.y = *reinterpret_cast<uint32_t*>(&hi);
-    *reinterpret_cast<uint2*>(a.out + ((size_t)b * rows_per_req + th) * kD + lane * 4) = pk;
-    if (a.lse && lane == 0) a.lse[(size_t)b * rows_per_req + th] = m2 + logf(tot);
 }
 
 // ---- host side ----------------------------------------------------------------------------------
@@ -697,44 +790,46 @@ int32_t encode(CUtensorMap* tm, const void* base, int rank, const cuuint64_t* di
 
 }  // namespace
 
-bool attn_prefix_tc_supported(const AttnPlan& pl) {
+bool attn_cascade_tc_supported(const AttnPlan& pl) {
     // contiguous KV only (paged KV stays on the mma.sync path), rows of one query tile must be whole
     // tree nodes (128 % G == 0), and the tensor-map extents must fit.
-    return pl.page_size == 0 && pl.d == kD && pl.G <= 128 && (128 % pl.G) == 0 && pl.kv_rows > 0 &&
-           pl.max_ctx_len > 0 && (int64_t)pl.B * pl.T_cap < (1ll << 31) && pl.kv_rows < (1ll << 31);
+    return pl.page_size == 0 && pl.d == kD && pl.G <= 128 && (128 % pl.G) == 0 &&
+           (int64_t)pl.B * pl.T_cap < (1ll << 31) && pl.kv_rows < (1ll << 31);
 }
 
-int32_t launch_attn_prefix_tc(const AttnPlan& pl, const AttnArgs& a, cudaStream_t s) {
+int32_t launch_attn_cascade_tc(const AttnPlan& pl, const AttnArgs& a, int mode, float* dbg_rows, cudaStream_t s) {
     static bool attr_set = false;
     if (!attr_set) {
-        D2SD_CHECK_CUDA(cudaFuncSetAttribute(attn_prefix_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        D2SD_CHECK_CUDA(cudaFuncSetAttribute(attn_cascade_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              (int)kSmemBytes));
         attr_set = true;
     }
-    CUtensorMap tm_q, tm_k, tm_v;
+    CUtensorMap tm_q, tm_k, tm_v, tm_tk, tm_tv;
     {   // Q [B*T_cap, Hq, d] viewed as (d_lo 64, hh G, t B*T_cap, d_hi 2, g Hkv): one box = one 128-row query tile
         const cuuint64_t dims[5] = {64, (cuuint64_t)pl.G, (cuuint64_t)pl.B * pl.T_cap, 2, (cuuint64_t)pl.Hkv};
         const cuuint64_t strides[4] = {(cuuint64_t)kD * 2, (cuuint64_t)pl.Hq * kD * 2, 128, (cuuint64_t)pl.G * kD * 2};
         const cuuint32_t box[5] = {64, (cuuint32_t)pl.G, (cuuint32_t)(kTileM / pl.G), 2, 1};
         if (int32_t st = encode(&tm_q, a.q, 5, dims, strides, box, "q")) return st;
     }
-    {   // K/V [kv_rows, Hkv, d] viewed as (d_lo 64, row, d_hi 2, g): one box = one 128-key tile
-        const cuuint64_t dims[4] = {64, (cuuint64_t)pl.kv_rows, 2, (cuuint64_t)pl.Hkv};
+    {   // K/V [rows, Hkv, d] viewed as (d_lo 64, row, d_hi 2, g): one box = one 128-key tile.  Rows past the
+        // end of the tensor are zero-filled by TMA; the kernel masks every key past a tile's valid count.
         const cuuint64_t strides[3] = {(cuuint64_t)pl.Hkv * kD * 2, 128, (cuuint64_t)kD * 2};
         const cuuint32_t box[4] = {64, kTileN, 2, 1};
-        if (int32_t st = encode(&tm_k, a.k_cache, 4, dims, strides, box, "k_cache")) return st;
-        if (int32_t st = encode(&tm_v, a.v_cache, 4, dims, strides, box, "v_cache")) return st;
+        const cuuint64_t tdims[4] = {64, (cuuint64_t)pl.B * pl.T_cap, 2, (cuuint64_t)pl.Hkv};
+        if (int32_t st = encode(&tm_tk, a.tree_k, 4, tdims, strides, box, "tree_k")) return st;
+        if (int32_t st = encode(&tm_tv, a.tree_v, 4, tdims, strides, box, "tree_v")) return st;
+        if (pl.kv_rows > 0 && a.k_cache && a.v_cache) {
+            const cuuint64_t dims[4] = {64, (cuuint64_t)pl.kv_rows, 2, (cuuint64_t)pl.Hkv};
+            if (int32_t st = encode(&tm_k, a.k_cache, 4, dims, strides, box, "k_cache")) return st;
+            if (int32_t st = encode(&tm_v, a.v_cache, 4, dims, strides, box, "v_cache")) return st;
+        } else {  // no committed prefix at all (max_ctx_len == 0): the maps are never used
+            tm_k = tm_tk;
+            tm_v = tm_tv;
+        }
     }
     dim3 grid(2 * pl.num_splits, pl.Hkv, pl.B * pl.n_mgroups);
-    attn_prefix_tc_kernel<<<grid, kThreads, kSmemBytes, s>>>(tm_q, tm_k, tm_v, pl, a);
-    D2SD_CHECK_LAUNCH("attn_prefix_tc_kernel");
-    return D2SD_OK;
-}
-
-int32_t launch_attn_merge_tc(const AttnPlan& pl, const AttnArgs& a, cudaStream_t s) {
-    const int rows = pl.B * pl.T_cap * pl.Hq;
-    attn_merge_tc_kernel<<<ceil_div(rows, 4), 128, 0, s>>>(pl, a);
-    D2SD_CHECK_LAUNCH("attn_merge_tc_kernel");
+    attn_cascade_tc_kernel<<<grid, kThreads, kSmemBytes, s>>>(tm_q, tm_k, tm_v, tm_tk, tm_tv, pl, a, mode, dbg_rows);
+    D2SD_CHECK_LAUNCH("attn_cascade_tc_kernel");
     return D2SD_OK;
 }
 

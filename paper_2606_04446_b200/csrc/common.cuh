@@ -66,9 +66,9 @@ int32_t launch_accept(const __nv_bfloat16* logits, int64_t row_stride, int V, co
 // Partial softmax states in the workspace.
 //  mma.sync path ("row layout"): O fp32 [B][NS][T_cap][Hq][d], LSE fp32 [B][NS][T_cap][Hq]; slots
 //    0..num_splits-1 are the prefix chunks, slot num_splits is the tree pass.
-//  tcgen05 path: prefix partials in the slot layout of attn_prefix_sm100.cu (O [B][NSLOT][Hkv]
-//    [rows_pad][d] with swizzled 16-byte chunks, LSE [B][NSLOT][Hkv][rows_pad], NSLOT = 2*num_splits);
-//    the tree state in the row layout with NS = 1 (tree_o [B][T_cap][Hq][d], tree_lse [B][T_cap][Hq]).
+//  tcgen05 path (attn_cascade_sm100.cu): a header of self-resetting group counters (zero between
+//    calls), then partials in the slot layout O [B][NSLOT][Hkv][rows_pad][d], LSE [B][NSLOT][Hkv]
+//    [rows_pad], NSLOT = 2*num_splits; the tree keys are key tiles of the same kernel.
 struct AttnPlan {
     int B, T_cap, W, Hq, Hkv, G, d;
     float sm_scale;
@@ -76,13 +76,13 @@ struct AttnPlan {
     int max_ctx_len;
     int64_t kv_rows;
     int num_splits;   // prefix chunks
-    int chunk_keys;   // keys per chunk (mma.sync: multiple of 64; tcgen05: multiple of 16)
+    int chunk_keys;   // mma.sync path: keys per chunk (multiple of 64); tcgen05 cuts whole key tiles on device
     int NS;           // row layout: num_splits + 1
     bool use_tc;      // tcgen05 prefix pass
     int n_mgroups;    // tcgen05: groups of <= 3 query tiles (384 rows) per kv head
     int rows_pad;     // tcgen05: n_mgroups * 384
     int NSLOT;        // tcgen05: 2 * num_splits
-    size_t off_o, off_lse, off_tree_o, off_tree_lse, bytes;
+    size_t off_cnt, cnt_bytes, off_o, off_lse, bytes;
 };
 
 struct AttnArgs {
@@ -92,14 +92,14 @@ struct AttnArgs {
     __nv_bfloat16* out;
     float *lse, *dbg_state;
     float *part_o, *part_lse;
-    float *tree_o, *tree_lse;  // tcgen05 path only
+    unsigned* counters;  // tcgen05 path only: [group][2] arrivals / done
 };
 
 int32_t launch_attn_mma(const AttnPlan& pl, const AttnArgs& a, bool do_prefix, bool do_tree,
                         cudaStream_t s);
 int32_t launch_attn_merge(const AttnPlan& pl, const AttnArgs& a, cudaStream_t s);
-int32_t launch_attn_prefix_tc(const AttnPlan& pl, const AttnArgs& a, cudaStream_t s);
-int32_t launch_attn_merge_tc(const AttnPlan& pl, const AttnArgs& a, cudaStream_t s);
-bool attn_prefix_tc_supported(const AttnPlan& pl);
+// mode: bit 0 = prefix tiles, bit 1 = tree tiles; dbg_rows: fp32 [B][T_cap][Hq][d+1] instead of out/lse
+int32_t launch_attn_cascade_tc(const AttnPlan& pl, const AttnArgs& a, int mode, float* dbg_rows, cudaStream_t s);
+bool attn_cascade_tc_supported(const AttnPlan& pl);
 
 }  // namespace d2sd

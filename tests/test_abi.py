@@ -27,7 +27,7 @@ def _declared_symbols():
 def test_library_exports_every_declared_symbol(d2sd):
     names = _declared_symbols()
     assert {"d2sd_select_prefixes", "d2sd_build_tree", "d2sd_cascade_verify_attn", "d2sd_accept",
-            "d2sd_cascade_workspace_bytes", "d2sd_accept_workspace_bytes", "d2sd_last_error",
+            "d2sd_cascade_workspace_bytes", "d2sd_cascade_workspace_init", "d2sd_accept_workspace_bytes", "d2sd_last_error",
             "d2sd_version"} <= set(names)
     L = ctypes.CDLL(d2sd.lib_path())
     for n in names:

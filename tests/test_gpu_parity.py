@@ -328,7 +328,7 @@ def test_graph_capture_whole_path(d2sd, oracle):
                            tree_ref["tree_len"])
     conf, d1, d2c, ctx = torch.from_numpy(st["conf"]).cuda(), i32_cuda(st["draft1"]), i32_cuda(st["draft2"]), i32_cuda(st["ctx_len"])
     q, kc, vc, tk, tv, lg = (bf16_cuda(x) for x in (ti["q"], kv["k_cache"], kv["v_cache"], ti["tree_k"], ti["tree_v"], logits))
-    ws = torch.empty(d2sd.cascade_workspace_bytes(cfg.B, cfg.T_cap, cfg.Hq, cfg.Hkv, cfg.d, 256, kv_rows=256), dtype=torch.uint8, device="cuda")
+    ws = d2sd.cascade_workspace(cfg.B, cfg.T_cap, cfg.Hq, cfg.Hkv, cfg.d, 256)
     ws2 = torch.empty(d2sd.accept_workspace_bytes(cfg.B, cfg.T_cap, cfg.V), dtype=torch.uint8, device="cuda")
     res = {}
 
