@@ -68,27 +68,53 @@ static int32_t make_plan(const d2sd_attn_params* p, AttnPlan* out) {
     const int max_ctx = p->max_ctx_len > 0 ? p->max_ctx_len : 1;
     int splits = p->num_splits;
     if (pl.use_tc) {
-        // One wave of CTA pairs (1 CTA/SM): a work item (request, kv head, group of <= 3 query tiles,
-        // chunk of key tiles) is served by two CTAs.  The key tiles of a request are its prefix tiles
-        // followed by its tree tiles; the kernel cuts them into num_splits chunks of whole tiles.
-        pl.n_mgroups = ceil_div(rows, 384);
-        pl.rows_pad = pl.n_mgroups * 384;
+        // Query tiles (2p, 2p+1) form pair items, an odd last tile the single item; every item gets its
+        // own run of context chunks (one CTA each).  A pair item does two units per key tile, a single
+        // item one, so the single item gets about half as many chunks.  With enough SMs for one wave the
+        // chunk counts fill the machine and every request cuts its own key tiles evenly (tps_min = 1);
+        // otherwise chunks have a fixed length and short requests simply use fewer of them.
+        const int n_mt = ceil_div(rows, 128);
+        pl.n_pair = n_mt / 2;
+        pl.n_single = n_mt & 1;
         const int max_tiles = ceil_div(p->max_ctx_len, 128) + ceil_div(pl.T_cap, 128);
-        if (splits == 0) {
-            const int64_t per_split = (int64_t)pl.B * pl.Hkv * pl.n_mgroups;
-            splits = (int)((sm_count() / 2) / (per_split > 0 ? per_split : 1));
-            if (splits > 64) splits = 64;
+        const int64_t heads = (int64_t)pl.B * pl.Hkv;
+        const int budget = (int)(sm_count() / (heads > 0 ? heads : 1));  // CTAs per (request, kv head), one wave
+        int ca, cb;
+        pl.tps_min = 1;
+        if (splits > 0) {
+            ca = splits;
+            cb = (splits + 1) / 2;
+        } else if (budget >= pl.n_pair + pl.n_single) {
+            ca = cb = 1;
+            if (pl.n_pair > 0) {
+                while (pl.n_pair * (ca + 1) + pl.n_single * ((ca + 2) / 2) <= budget) ++ca;
+                cb = (ca + 1) / 2;
+                if (pl.n_single) cb = (budget - pl.n_pair * ca) / pl.n_single;
+            } else {
+                cb = budget;
+            }
+        } else {
+            ca = ceil_div(max_tiles, 32);
+            cb = ceil_div(max_tiles, 64);
+            pl.tps_min = -1;  // fixed below
         }
-        if (splits > 64) splits = 64;                // a group's 2*splits CTAs wait for each other: one wave
-        if (splits > max_tiles) splits = max_tiles;  // never an always-empty chunk
-        if (splits < 1) splits = 1;
+        if (ca > 64) ca = 64;  // a group's CTAs wait for each other
+        if (cb > 64) cb = 64;
+        if (ca > max_tiles) ca = max_tiles;  // never an always-empty chunk
+        if (cb > max_tiles) cb = max_tiles;
+        if (ca < 1) ca = 1;
+        if (cb < 1) cb = 1;
+        if (pl.tps_min < 0) pl.tps_min = ceil_div(max_tiles, pl.n_pair ? ca : cb);
+        pl.chunks_a = ca;
+        pl.chunks_b = cb;
         pl.chunk_keys = 0;
-        pl.num_splits = splits;
-        pl.NSLOT = 2 * pl.num_splits;
+        pl.num_splits = pl.n_pair ? ca : cb;
         pl.NS = 0;
-        const size_t slot_rows = (size_t)pl.B * pl.NSLOT * pl.Hkv * pl.rows_pad;
+        pl.grp_rows = 256 * (pl.n_pair ? (pl.n_single && cb > ca ? cb : ca) : cb);
+        const size_t n_groups = (size_t)pl.B * pl.Hkv * (pl.n_pair + pl.n_single);
+        const size_t slot_rows = n_groups * pl.grp_rows;
         pl.off_cnt = 0;
-        pl.cnt_bytes = align_up((size_t)pl.B * pl.Hkv * pl.n_mgroups * 2 * sizeof(unsigned), 256);
+        pl.cnt_bytes = align_up(n_groups * 2 * sizeof(unsigned), 256);
         pl.off_o = pl.cnt_bytes;
         pl.off_lse = pl.off_o + align_up(slot_rows * pl.d * sizeof(float), 256);
         pl.bytes = pl.off_lse + align_up(slot_rows * sizeof(float), 256);

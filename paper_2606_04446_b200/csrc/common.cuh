@@ -67,8 +67,10 @@ int32_t launch_accept(const __nv_bfloat16* logits, int64_t row_stride, int V, co
 //  mma.sync path ("row layout"): O fp32 [B][NS][T_cap][Hq][d], LSE fp32 [B][NS][T_cap][Hq]; slots
 //    0..num_splits-1 are the prefix chunks, slot num_splits is the tree pass.
 //  tcgen05 path (attn_cascade_sm100.cu): a header of self-resetting group counters (zero between
-//    calls), then partials in the slot layout O [B][NSLOT][Hkv][rows_pad][d], LSE [B][NSLOT][Hkv]
-//    [rows_pad], NSLOT = 2*num_splits; the tree keys are key tiles of the same kernel.
+//    calls), then partials per group (request, kv head, item): O fp32 [group][grp_rows][d] and LSE
+//    fp32 [group][grp_rows]; a pair item holds chunk c's two query tiles at rows c*256.., a single
+//    item holds (chunk c, key-tile parity s) at rows (2c+s)*128..; the tree keys are key tiles of
+//    the same kernel.
 struct AttnPlan {
     int B, T_cap, W, Hq, Hkv, G, d;
     float sm_scale;
@@ -79,9 +81,12 @@ struct AttnPlan {
     int chunk_keys;   // mma.sync path: keys per chunk (multiple of 64); tcgen05 cuts whole key tiles on device
     int NS;           // row layout: num_splits + 1
     bool use_tc;      // tcgen05 prefix pass
-    int n_mgroups;    // tcgen05: groups of <= 3 query tiles (384 rows) per kv head
-    int rows_pad;     // tcgen05: n_mgroups * 384
-    int NSLOT;        // tcgen05: 2 * num_splits
+    // tcgen05: the query rows (T*G) of one kv head are cut into 128-row tiles; tiles (2p, 2p+1) form
+    // "pair item" p, an odd last tile is the "single item".  Item kinds get their own chunk counts.
+    int n_pair, n_single;    // items per (request, kv head), from T_cap
+    int chunks_a, chunks_b;  // CTAs (context chunks) per pair item / per single item
+    int tps_min;             // a chunk never holds fewer key tiles than this (unless the request ends)
+    int grp_rows;            // partial-state rows per group: max(chunks_a*256, chunks_b*256)
     size_t off_cnt, cnt_bytes, off_o, off_lse, bytes;
 };
 
