@@ -26,7 +26,8 @@
 //
 // TMEM (512 columns): O_0, O_1 (128 fp32 columns each), S_0/P_0, S_1/P_1 (128 each).
 // Warp roles (384 threads): warps 0..3 = softmax team 0, warps 4..7 = team 1, warp 8 = TMA producer,
-// warp 9 = MMA issuer (one thread), warp 10 = TMEM allocator, warp 11 = zeroes the V rows behind a
+// warps 9 / 10 = MMA issuers of slot 0 / 1 (one thread each; warp 10 also owns the TMEM allocation),
+// warp 11 = zeroes the V rows behind a
 // ragged tile end (they are multiplied by exact zeros and may hold anything, NaN included).  The
 // control warps have the HIGHEST warp ids on purpose: the SM's issue arbiter prefers higher warp ids,
 // and a starved MMA issuer stalls the whole pipeline while the softmax warps always have work.  The
@@ -264,6 +265,13 @@ __device__ __forceinline__ uint32_t pack2_bf16(float lo, float hi) {
     return *reinterpret_cast<uint32_t*>(&v);
 }
 
+// One lane of a fully active warp; unlike `lane == 0` it lets ptxas keep the MMA operands on the uniform
+// datapath (no per-instruction elect loop around every tcgen05.mma).
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+    return pred != 0;
+}
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 // shared -> global bulk copy (bytes % 16 == 0), one bulk group per call site
@@ -283,8 +291,11 @@ __device__ long long g_timeline[256][128];
         const int _c = blockIdx.x + gridDim.x * blockIdx.y;                                         \
         if (_c < 256 && (slot) < 128) g_timeline[_c][(slot)] = clock64() - tl_t0;                   \
     } while (0)
+// accumulate the cycles since the previous TLA of this thread into bucket `b` (dumped at slots 3..15)
+#define TLA(b) do { const long long _t = clock64(); tl_acc[(b)] += _t - tl_last; tl_last = _t; } while (0)
 #else
 #define TL(slot) do {} while (0)
+#define TLA(b) do {} while (0)
 #endif
 
 // What one CTA does: which item / chunk, which rows its two slots hold, which key tiles it streams.
@@ -415,13 +426,13 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
         mbar_init(bar(kBarQFull + 1), 1);
         for (int i = 0; i < kRing; ++i) {
             mbar_init(bar(kBarFull + i), 1);
-            mbar_init(bar(kBarEmpty + i), 2);  // the MMA's commit + the V sanitiser
+            mbar_init(bar(kBarEmpty + i), 3);  // the two MMA issuers' commits + the V sanitiser
         }
         for (int s = 0; s < 2; ++s) {
             mbar_init(bar(kBarSFull + s), 1);
             for (int q = 0; q < 4; ++q) mbar_init(bar(kBarPFull + 4 * s + q), kTileM);
         }
-        mbar_init(bar(kBarAllDone), 1);
+        mbar_init(bar(kBarAllDone), 2);
         mbar_init(bar(kBarVFix + 0), 1);
         mbar_init(bar(kBarVFix + 1), 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -506,7 +517,7 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
         // fall through to the TMEM release
       } else if (warp == 8) {
         // ===== TMA producer: K_0 first (the first MMA needs it), then the Q tiles, then the ring =====
-        if (lane == 0) {
+        if (elect_one()) {
             int x = 0;  // ring position of the next tile to load
             for (int jj = 0; jj < wk.n_tiles; ++jj) {
                 const TileInfo ti = tile_info(jj);
@@ -530,80 +541,96 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 }
             }
         }
-      } else if (warp == 9) {
-        // ===== MMA issuer (one thread).  Q.K^T of the next unit is issued before P.V of the previous
-        // one whenever they use different S buffers (slots), so the tensor pipe works on the next S
-        // while a softmax team turns the previous S into P. =====
-        if (lane == 0) {
-            const bool one_q = wk.mode != kModePair;
-            const uint64_t qd0 = smem_desc(smem + kOffQ, 16, 1024);
-            const uint64_t qd1 = smem_desc(smem + kOffQ + (one_q ? 0u : kQTileBytes), 16, 1024);
-            uint32_t qk_started = 0, pv_started = 0, pv_par = 0;  // bit s: per-slot flags / phase parity
-            bool pend = false, pend_last = false, pend_first = false, pend_ragged = false;
-            int pend_slot = 0, pend_vx = 0, pend_n = 0, n_ragged = 0, n = 0;
-            auto do_pv = [&]() {
-                const int s = pend_slot, vi = pend_vx % kRing;
-                if (pend_first) {  // first P.V on this V tile
-                    mbar_wait(bar(kBarFull + vi), (pend_vx / kRing) & 1);
-                    if (pend_ragged) mbar_wait(bar(kBarVFix + n_ragged++), 0);
-                }
-                const uint64_t vd = smem_desc(smem + kOffRing + vi * kKvTileBytes, kKvTileBytes / 2, 1024);
-                const uint32_t pa = tmem + kTmemS + s * kTileN;
-                const uint32_t od = tmem + s * kD;
-                const int ksteps = pend_n >> 4;
-                // P arrives in four 32-key pieces (two K steps each); piece 0 is always waited for, and
-                // its arrival implies that every piece of the previous unit has completed its phase
-#pragma unroll 1
-                for (int q = 0; 2 * q < ksteps; ++q) {
-                    mbar_wait(bar(kBarPFull + 4 * s + q), (pv_par >> s) & 1u);
-                    tc_fence_after();
-                    for (int ks = 2 * q; ks < min(2 * q + 2, ksteps); ++ks)
-                        umma_ts(od, pa + ks * 8, vd + (uint64_t)(ks * (2048 >> 4)), kIdescPV,
-                                (((pv_started >> s) & 1u) | ks) != 0);
-                }
-                if (pend_last) tc_commit(bar(kBarEmpty + vi));
-                pv_started |= 1u << s;
-                pv_par ^= 1u << s;
-                pend = false;
-            };
+      } else if (warp == 9 || warp == 10) {
+        // ===== MMA issuers: one elected thread per SLOT (warp 9 -> slot 0, warp 10 -> slot 1).  The two
+        // slots' chains (Q.K^T -> softmax -> P.V -> next Q.K^T) are independent, so each thread simply
+        // walks its own chain; the tensor pipe interleaves them, and the single-thread issue cost
+        // (barrier waits, commits, 16 MMAs per unit) of one slot hides behind the other slot's work.
+        // Both threads release every ring tile (a thread that does not use a tile commits at once). =====
+        if (elect_one()) {
+            const int s = warp - 9;
+            const bool slot_used = wk.mode != kModeSolo || s == 0;
+            const uint64_t qd = smem_desc(smem + kOffQ + (wk.mode == kModePair && s ? kQTileBytes : 0u), 16, 1024);
+            const uint32_t sd = tmem + kTmemS + s * kTileN;  // S, overwritten by P (bf16, 64 columns)
+            const uint32_t od = tmem + s * kD;
+            uint32_t acc = 0, par = 0, n_ragged = 0;
+            bool q_ready = false;
+#ifdef D2SD_TIMELINE
+            long long tl_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0}, tl_last = clock64();
+            int n = 0;
+#endif
+            int ki = 0, kpar = 0;  // ring slot / fill parity of the tile being consumed (K_j, then V_j)
             for (int jj = 0; jj < wk.n_tiles; ++jj) {
-                const int kx = 2 * jj, vx = 2 * jj + 1;
-                const int ki = kx % kRing;
+                const bool used = slot_used && ((wk.uses(jj) >> s) & 1u);
                 const int valid = tile_info(jj).valid;
                 const int tile_n = (valid + 15) & ~15;  // MMA N of Q.K^T and K extent of P.V (multiple of 16)
-                const uint32_t use = wk.uses(jj);
-                mbar_wait(bar(kBarFull + ki), (kx / kRing) & 1);
-                const uint64_t kd = smem_desc(smem + kOffRing + ki * kKvTileBytes, 16, 1024);
-                const uint32_t id_qk = idesc(kTileM, (uint32_t)tile_n, 0);
-                for (int s = 0; s < 2; ++s) {
-                    if (!((use >> s) & 1u)) continue;
-                    const bool first_of_tile = (use & ((1u << s) - 1u)) == 0;
-                    const bool last_of_tile = (use >> (s + 1)) == 0;
-                    if (pend && pend_slot == s) do_pv();  // same S buffer: P must be consumed first
-                    if (!((qk_started >> s) & 1u)) mbar_wait(bar(kBarQFull + (one_q ? 0 : s)), 0);
-                    TL(16 + 3 * n);
+                const bool ragged = (valid & 15) != 0;
+                // ---- S = Q . K_j^T ----
+                if (used) {
+                    TLA(0);
+                    mbar_wait(bar(kBarFull + ki), kpar);
+                    if (!q_ready) {
+                        mbar_wait(bar(kBarQFull + (wk.mode == kModePair ? s : 0)), 0);
+                        q_ready = true;
+                    }
+                    TLA(5);  // K wait
+#ifdef D2SD_TIMELINE
+                    if (n < 8) TL(16 + 6 * n + 3 * s);
+#endif
                     tc_fence_after();
-                    const uint32_t sd = tmem + kTmemS + s * kTileN;
+                    const uint64_t kd = smem_desc(smem + kOffRing + ki * kKvTileBytes, 16, 1024);
+                    const uint32_t id_qk = idesc(kTileM, (uint32_t)tile_n, 0);
 #pragma unroll
                     for (int kk = 0; kk < kD / 16; ++kk) {
                         const uint64_t off = (uint64_t)(((kk >> 2) * (kQTileBytes / 2) + (kk & 3) * 32) >> 4);
-                        umma_ss(sd, (s ? qd1 : qd0) + off, kd + off, id_qk, kk > 0);
+                        umma_ss(sd, qd + off, kd + off, id_qk, kk > 0);
                     }
+                    TLA(6);  // Q.K^T issue
                     tc_commit(bar(kBarSFull + s));
-                    if (last_of_tile) tc_commit(bar(kBarEmpty + ki));
-                    qk_started |= 1u << s;
-                    if (pend) {
-                        do_pv();
-                        TL(16 + 3 * (n - 1) + 2);
-                    }
-                    pend = true; pend_slot = s; pend_vx = vx; pend_n = tile_n;
-                    pend_first = first_of_tile; pend_last = last_of_tile;
-                    pend_ragged = (valid & 15) != 0;
-                    ++n;
                 }
+                tc_commit(bar(kBarEmpty + ki));
+                TLA(4);
+                if (++ki == kRing) { ki = 0; kpar ^= 1; }
+                // ---- O += P . V_j, P released by the softmax team in four 32-key pieces ----
+                if (used) {
+                    mbar_wait(bar(kBarFull + ki), kpar);
+                    if (ragged) mbar_wait(bar(kBarVFix + n_ragged), 0);
+                    TLA(1);  // V wait
+                    const uint64_t vd = smem_desc(smem + kOffRing + ki * kKvTileBytes, kKvTileBytes / 2, 1024);
+                    const int ksteps = tile_n >> 4;
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        if (2 * q < ksteps) {
+                            mbar_wait(bar(kBarPFull + 4 * s + q), par);
+                            TLA(2);  // P wait
+                            tc_fence_after();
+#pragma unroll
+                            for (int ks = 2 * q; ks < 2 * q + 2; ++ks)
+                                if (ks < ksteps)
+                                    umma_ts(od, sd + ks * 8, vd + (uint64_t)(ks * (2048 >> 4)), kIdescPV, acc | ks);
+                            TLA(3);  // P.V issue
+                        }
+                    }
+                    acc = 1;
+                    par ^= 1;
+#ifdef D2SD_TIMELINE
+                    if (n < 8) TL(16 + 6 * n + 3 * s + 2);
+                    ++n;
+#endif
+                }
+                if (ragged) ++n_ragged;
+                tc_commit(bar(kBarEmpty + ki));
+                TLA(4);
+                if (++ki == kRing) { ki = 0; kpar ^= 1; }
             }
-            if (pend) do_pv();
             tc_commit(bar(kBarAllDone));
+#ifdef D2SD_TIMELINE
+            TLA(0);
+            for (int i = 0; i < 7; ++i) {
+                const int _c = blockIdx.x + gridDim.x * blockIdx.y;
+                if (_c < 256 && s == 0) g_timeline[_c][3 + i] = tl_acc[i];
+            }
+#endif
         }
       } else if (warp == 11) {
         // ===== V sanitiser: the P.V MMA runs over ceil16(valid) keys; rows valid..ceil16(valid)-1 of a
@@ -650,7 +677,11 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
         const float thr = kRescaleThreshold / c2;  // in raw score units
         const bool slot_used = wk.mode != kModeSolo || s == 0;
         const int rows_s = wk.rows(s);
+#ifdef D2SD_DBG_NOSOFTMAX
+        const bool warp_active = false;  // timing experiment only: results are garbage
+#else
         const bool warp_active = slot_used && w * 32 < rows_s;
+#endif
         const uint32_t sbuf = tmem + kTmemS + s * kTileN + lane_addr;
         const uint32_t o_addr = tmem + s * kD + lane_addr;
         float m_run = -INFINITY, l_run = 0.f;
@@ -661,7 +692,7 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 const TileInfo ti = tile_info(jj);
                 const bool masked_tile = ti.tree || ti.valid < kTileN;
                 mbar_wait(bar(kBarSFull + s), k & 1);
-                if (w == 0 && lane == 0) TL(64 + 4 * k + 2 * s);
+                if (w == 0 && lane == 0 && k < 8) TL(64 + 4 * k + 2 * s);
                 if (warp_active) {
                     uint32_t sv[128];
                     tc_fence_after();
@@ -748,7 +779,7 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
 #pragma unroll
                     for (int q = 0; q < 4; ++q) mbar_arrive(bar(kBarPFull + 4 * s + q));
                 }
-                if (w == 0 && lane == 0) TL(64 + 4 * k + 2 * s + 1);
+                if (w == 0 && lane == 0 && k < 8) TL(64 + 4 * k + 2 * s + 1);
                 ++k;
             }
         }
