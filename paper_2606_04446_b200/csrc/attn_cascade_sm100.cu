@@ -141,6 +141,9 @@ __device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* tm) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(tm)) : "memory");
 }
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void named_bar_arrive(uint32_t id, uint32_t threads) {
+    asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(threads) : "memory");
+}
 __device__ __forceinline__ void named_bar_sync(uint32_t id, uint32_t threads) {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
 }
@@ -258,6 +261,13 @@ __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.
 __device__ __forceinline__ float ex2(float x) {
     float y;
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+// Same, but ordered against the other volatile statements (TMEM stores / waits, barrier arrivals): the
+// softmax loop uses it to keep a piece's exponentials ahead of the wait for the previous piece's store.
+__device__ __forceinline__ float ex2_ordered(float x) {
+    float y;
+    asm volatile("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
 __device__ __forceinline__ uint32_t pack2_bf16(float lo, float hi) {
@@ -544,9 +554,11 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
       } else if (warp == 9 || warp == 10) {
         // ===== MMA issuers: one elected thread per SLOT (warp 9 -> slot 0, warp 10 -> slot 1).  The two
         // slots' chains (Q.K^T -> softmax -> P.V -> next Q.K^T) are independent, so each thread simply
-        // walks its own chain; the tensor pipe interleaves them, and the single-thread issue cost
-        // (barrier waits, commits, 16 MMAs per unit) of one slot hides behind the other slot's work.
-        // Both threads release every ring tile (a thread that does not use a tile commits at once). =====
+        // walks its own chain and the tensor pipe interleaves them.  The chain's tensor phase is kept
+        // short: the next unit's K tile is waited for BEFORE the P pieces, and the next Q.K^T is issued
+        // right behind the last P.V piece (S and P share TMEM columns, so it cannot go earlier).
+        // Both threads release every ring tile; a tile the slot does not use is released as soon as
+        // its fill has been observed (so the arrival can only count for that fill). =====
         if (elect_one()) {
             const int s = warp - 9;
             const bool slot_used = wk.mode != kModeSolo || s == 0;
@@ -554,74 +566,104 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             const uint32_t sd = tmem + kTmemS + s * kTileN;  // S, overwritten by P (bf16, 64 columns)
             const uint32_t od = tmem + s * kD;
             uint32_t acc = 0, par = 0, n_ragged = 0;
-            bool q_ready = false;
 #ifdef D2SD_TIMELINE
             long long tl_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0}, tl_last = clock64();
             int n = 0;
 #endif
-            int ki = 0, kpar = 0;  // ring slot / fill parity of the tile being consumed (K_j, then V_j)
-            for (int jj = 0; jj < wk.n_tiles; ++jj) {
-                const bool used = slot_used && ((wk.uses(jj) >> s) & 1u);
-                const int valid = tile_info(jj).valid;
-                const int tile_n = (valid + 15) & ~15;  // MMA N of Q.K^T and K extent of P.V (multiple of 16)
-                const bool ragged = (valid & 15) != 0;
-                // ---- S = Q . K_j^T ----
-                if (used) {
-                    TLA(0);
-                    mbar_wait(bar(kBarFull + ki), kpar);
-                    if (!q_ready) {
-                        mbar_wait(bar(kBarQFull + (wk.mode == kModePair ? s : 0)), 0);
-                        q_ready = true;
+            int jj = 0, ki = 0, kpar = 0;  // current tile and the ring slot / fill parity of its K
+            auto ring_next = [&](int& i, int& p) { if (++i == kRing) { i = 0; p ^= 1; } };
+            auto is_used = [&](int j) { return slot_used && ((wk.uses(j) >> s) & 1u); };
+            auto valid_of = [&](int j) { return tile_info(j).valid; };
+            // Walk from tile nj to the slot's next used tile: an unused tile is released once its fills
+            // have been observed; at a used tile, its K fill is awaited.  Non-blocking mode gives up at the
+            // first fill that has not landed yet (returns false) and can be resumed.
+            int nj = 0, nki = 0, nkpar = 0, nsub = 0;
+            auto advance = [&](bool blocking) {
+                while (nj < wk.n_tiles) {
+                    if (is_used(nj)) {
+                        if (blocking) mbar_wait(bar(kBarFull + nki), nkpar);
+                        else if (!mbar_try_wait(bar(kBarFull + nki), nkpar)) return false;
+                        return true;
                     }
-                    TLA(5);  // K wait
-#ifdef D2SD_TIMELINE
-                    if (n < 8) TL(16 + 6 * n + 3 * s);
-#endif
-                    tc_fence_after();
-                    const uint64_t kd = smem_desc(smem + kOffRing + ki * kKvTileBytes, 16, 1024);
-                    const uint32_t id_qk = idesc(kTileM, (uint32_t)tile_n, 0);
-#pragma unroll
-                    for (int kk = 0; kk < kD / 16; ++kk) {
-                        const uint64_t off = (uint64_t)(((kk >> 2) * (kQTileBytes / 2) + (kk & 3) * 32) >> 4);
-                        umma_ss(sd, qd + off, kd + off, id_qk, kk > 0);
+                    while (nsub < 2) {
+                        if (blocking) mbar_wait(bar(kBarFull + nki), nkpar);
+                        else if (!mbar_try_wait(bar(kBarFull + nki), nkpar)) return false;
+                        tc_commit(bar(kBarEmpty + nki));
+                        ring_next(nki, nkpar);
+                        ++nsub;
                     }
-                    TLA(6);  // Q.K^T issue
-                    tc_commit(bar(kBarSFull + s));
+                    if (valid_of(nj) & 15) ++n_ragged;
+                    nsub = 0;
+                    ++nj;
                 }
-                tc_commit(bar(kBarEmpty + ki));
-                TLA(4);
-                if (++ki == kRing) { ki = 0; kpar ^= 1; }
-                // ---- O += P . V_j, P released by the softmax team in four 32-key pieces ----
-                if (used) {
-                    mbar_wait(bar(kBarFull + ki), kpar);
-                    if (ragged) mbar_wait(bar(kBarVFix + n_ragged), 0);
-                    TLA(1);  // V wait
-                    const uint64_t vd = smem_desc(smem + kOffRing + ki * kKvTileBytes, kKvTileBytes / 2, 1024);
-                    const int ksteps = tile_n >> 4;
+                return true;
+            };
+            auto issue_qk = [&](int j, int i) {
+                const int tile_n = (valid_of(j) + 15) & ~15;  // MMA N (multiple of 16)
+                const uint64_t kd = smem_desc(smem + kOffRing + i * kKvTileBytes, 16, 1024);
+                const uint32_t id_qk = idesc(kTileM, (uint32_t)tile_n, 0);
+                tc_fence_after();
 #pragma unroll
-                    for (int q = 0; q < 4; ++q) {
-                        if (2 * q < ksteps) {
-                            mbar_wait(bar(kBarPFull + 4 * s + q), par);
-                            TLA(2);  // P wait
-                            tc_fence_after();
-#pragma unroll
-                            for (int ks = 2 * q; ks < 2 * q + 2; ++ks)
-                                if (ks < ksteps)
-                                    umma_ts(od, sd + ks * 8, vd + (uint64_t)(ks * (2048 >> 4)), kIdescPV, acc | ks);
-                            TLA(3);  // P.V issue
-                        }
-                    }
-                    acc = 1;
-                    par ^= 1;
-#ifdef D2SD_TIMELINE
-                    if (n < 8) TL(16 + 6 * n + 3 * s + 2);
-                    ++n;
-#endif
+                for (int kk = 0; kk < kD / 16; ++kk) {
+                    const uint64_t off = (uint64_t)(((kk >> 2) * (kQTileBytes / 2) + (kk & 3) * 32) >> 4);
+                    umma_ss(sd, qd + off, kd + off, id_qk, kk > 0);
                 }
-                if (ragged) ++n_ragged;
-                tc_commit(bar(kBarEmpty + ki));
+                tc_commit(bar(kBarSFull + s));
+                tc_commit(bar(kBarEmpty + i));  // K_j is free once this Q.K^T has completed
+            };
+            advance(true);
+            jj = nj; ki = nki; kpar = nkpar;
+            if (jj < wk.n_tiles) {
+                mbar_wait(bar(kBarQFull + (wk.mode == kModePair ? s : 0)), 0);
+                TLA(5);
+#ifdef D2SD_TIMELINE
+                TL(16 + 3 * s);
+#endif
+                issue_qk(jj, ki);
+                TLA(6);
+            }
+            while (jj < wk.n_tiles) {
+                const int valid = valid_of(jj);
+                const int ksteps = ((valid + 15) & ~15) >> 4;  // K extent of P.V in 16-key steps
+                int vi = ki, vpar = kpar;
+                ring_next(vi, vpar);
+                mbar_wait(bar(kBarFull + vi), vpar);
+                if (valid & 15) mbar_wait(bar(kBarVFix + n_ragged++), 0);
+                TLA(1);  // V wait
+                // the next unit of this slot and its K tile, before the P pieces arrive
+                nj = jj + 1; nki = vi; nkpar = vpar; nsub = 0;
+                ring_next(nki, nkpar);
+                const bool next_ready = advance(false);
+                TLA(5);  // K wait
+                const uint64_t vd = smem_desc(smem + kOffRing + vi * kKvTileBytes, kKvTileBytes / 2, 1024);
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    if (2 * q < ksteps) {
+                        mbar_wait(bar(kBarPFull + 4 * s + q), par);
+                        TLA(2);  // P wait
+                        tc_fence_after();
+#pragma unroll
+                        for (int ks = 2 * q; ks < 2 * q + 2; ++ks)
+                            if (ks < ksteps) umma_ts(od, sd + ks * 8, vd + (uint64_t)(ks * (2048 >> 4)), kIdescPV, acc | ks);
+                    }
+                }
+                acc = 1;
+                par ^= 1;
+                TLA(3);  // P.V issue
+#ifdef D2SD_TIMELINE
+                if (n < 8) TL(16 + 6 * n + 3 * s + 2);
+                ++n;
+#endif
+                if (!next_ready) advance(true);
+                TLA(5);
+#ifdef D2SD_TIMELINE
+                if (nj < wk.n_tiles && n < 8) TL(16 + 6 * n + 3 * s);
+#endif
+                if (nj < wk.n_tiles) issue_qk(nj, nki);
+                TLA(6);  // Q.K^T issue
+                tc_commit(bar(kBarEmpty + vi));
                 TLA(4);
-                if (++ki == kRing) { ki = 0; kpar ^= 1; }
+                jj = nj; ki = nki; kpar = nkpar;
             }
             tc_commit(bar(kBarAllDone));
 #ifdef D2SD_TIMELINE
@@ -686,6 +728,11 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
         const uint32_t o_addr = tmem + s * kD + lane_addr;
         float m_run = -INFINITY, l_run = 0.f;
         int k = 0;  // units of this slot so far
+        // The exponentials of a unit saturate the SM's MUFU pipe, so the two teams take turns at them
+        // (named barriers 2 / 3, one hands the turn to the other): team 0's exp phase then overlaps team
+        // 1's tensor phase and vice versa instead of both teams computing and both waiting in step.
+        const bool pingpong = wk.mode != kModeSolo;
+        if (pingpong && s == 1) named_bar_arrive(2, 256);  // team 0 goes first
         if (slot_used) {
             for (int jj = 0; jj < wk.n_tiles; ++jj) {
                 if (!((wk.uses(jj) >> s) & 1u)) continue;
@@ -693,14 +740,16 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 const bool masked_tile = ti.tree || ti.valid < kTileN;
                 mbar_wait(bar(kBarSFull + s), k & 1);
                 if (w == 0 && lane == 0 && k < 8) TL(64 + 4 * k + 2 * s);
+                uint32_t sv[128];
+                float ms = 0.f;
                 if (warp_active) {
-                    uint32_t sv[128];
                     tc_fence_after();
                     D2SD_TMEM_LD32(sbuf, sv, 0);
                     D2SD_TMEM_LD32(sbuf + 32, sv, 32);
                     D2SD_TMEM_LD32(sbuf + 64, sv, 64);
                     D2SD_TMEM_LD32(sbuf + 96, sv, 96);
                     tmem_wait_ld();
+                    if (w == 0 && lane == 0 && k == 3) TL(102 + 8 * s);
                     if (masked_tile) {
                         // keys past the tile's end, and (tree tiles) keys that are not ancestors-or-self of
                         // this row's node: the tile's 128 mask bits -> -inf
@@ -751,33 +800,48 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                         }
                     }
                     // a row with every key so far masked has m_run = -inf: exp2(-inf - 0) = 0, not NaN
-                    const float ms = m_run == -INFINITY ? 0.f : m_run * c2;
+                    ms = m_run == -INFINITY ? 0.f : m_run * c2;
+                    if (w == 0 && lane == 0 && k == 3) TL(103 + 8 * s);
+                }
+                if (pingpong) named_bar_sync(2 + s, 256);  // this team's turn at the exponentials
+                if (w == 0 && lane == 0 && k == 3) TL(104 + 8 * s);
+                if (warp_active) {
                     float sum0 = 0.f, sum1 = 0.f;
+                    // P[128 x 128] bf16 = 64 TMEM columns, released 16 at a time.  The store of piece q is
+                    // only waited for after the exponentials of piece q+1 have been issued, so the MUFU
+                    // pipe never idles behind a TMEM store.
 #pragma unroll
-                    for (int q = 0; q < 4; ++q) {  // P[128 x 128] bf16 = 64 TMEM columns, released 16 at a time
+                    for (int q = 0; q < 4; ++q) {
+                        float ev[32];
+#pragma unroll
+                        for (int c = 0; c < 32; ++c) ev[c] = ex2_ordered(__uint_as_float(sv[q * 32 + c]) * c2 - ms);
+                        if (q > 0) {  // piece q-1 has landed in TMEM long ago: release it
+                            tmem_wait_st();
+                            tc_fence_before();
+                            mbar_arrive(bar(kBarPFull + 4 * s + q - 1));
+                        }
                         uint32_t p[16];
+                        float t0 = 0.f, t1 = 0.f, t2 = 0.f, t3 = 0.f;
 #pragma unroll
                         for (int c = 0; c < 16; c += 2) {
-                            const int e = q * 32 + 2 * c;
-                            const float e0 = ex2(__uint_as_float(sv[e]) * c2 - ms);
-                            const float e1 = ex2(__uint_as_float(sv[e + 1]) * c2 - ms);
-                            const float e2 = ex2(__uint_as_float(sv[e + 2]) * c2 - ms);
-                            const float e3 = ex2(__uint_as_float(sv[e + 3]) * c2 - ms);
-                            sum0 += e0 + e1;
-                            sum1 += e2 + e3;
-                            p[c] = pack2_bf16(e0, e1);
-                            p[c + 1] = pack2_bf16(e2, e3);
+                            t0 += ev[2 * c]; t1 += ev[2 * c + 1]; t2 += ev[2 * c + 2]; t3 += ev[2 * c + 3];
+                            p[c] = pack2_bf16(ev[2 * c], ev[2 * c + 1]);
+                            p[c + 1] = pack2_bf16(ev[2 * c + 2], ev[2 * c + 3]);
                         }
+                        sum0 += t0 + t1;
+                        sum1 += t2 + t3;
                         D2SD_TMEM_ST16(sbuf + q * 16, p);
-                        tmem_wait_st();
-                        tc_fence_before();
-                        mbar_arrive(bar(kBarPFull + 4 * s + q));
-                        if (q < 3) D2SD_PIN32(sv, (q + 1) * 32);
                     }
+                    if (w == 0 && lane == 0 && k == 3) TL(105 + 8 * s);
+                    if (pingpong) named_bar_arrive(3 - s, 256);  // exponentials issued: hand the turn over
                     l_run += sum0 + sum1;
+                    tmem_wait_st();
+                    tc_fence_before();
+                    mbar_arrive(bar(kBarPFull + 4 * s + 3));
                 } else {
 #pragma unroll
                     for (int q = 0; q < 4; ++q) mbar_arrive(bar(kBarPFull + 4 * s + q));
+                    if (pingpong) named_bar_arrive(3 - s, 256);
                 }
                 if (w == 0 && lane == 0 && k < 8) TL(64 + 4 * k + 2 * s + 1);
                 ++k;
