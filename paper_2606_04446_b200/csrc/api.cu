@@ -87,8 +87,10 @@ static int32_t make_plan(const d2sd_attn_params* p, AttnPlan* out) {
         } else if (budget >= pl.n_pair + pl.n_single) {
             ca = cb = 1;
             if (pl.n_pair > 0) {
-                while (pl.n_pair * (ca + 1) + pl.n_single * ((ca + 2) / 2) <= budget) ++ca;
-                cb = (ca + 1) / 2;
+                // measured unit costs: a single item's units cost ~0.65 of a pair item's two (they are
+                // tensor-bound but fetch a whole K/V tile per unit), so cb : ca ~ 0.65
+                while (pl.n_pair * (ca + 1) + pl.n_single * ((13 * (ca + 1) + 10) / 20) <= budget) ++ca;
+                cb = (13 * ca + 10) / 20;
                 if (pl.n_single) cb = (budget - pl.n_pair * ca) / pl.n_single;
             } else {
                 cb = budget;

@@ -16,8 +16,9 @@
 //   single item : both slots hold the same M tile; slot s takes the chunk's key tiles of parity s
 //                 (two running softmax states over disjoint keys, merged like any two chunks)
 //
-// so that two independent softmax teams (one warpgroup per slot, one thread per query row) work
-// phase-shifted: while team 0 turns S_0 into P_0, the tensor pipe computes S_1 and O_0 += P_0.V.
+// so that the tensor phase of one slot (P.V, then the next Q.K^T, which cannot start earlier because P
+// overwrites S in TMEM) runs under the other slot's softmax.  The eight softmax warps serve one unit
+// at a time, two threads per query row.
 // Per unit:
 //
 //   S[128 x 128] = Q_m[128 x 128] . K_j^T    tcgen05.mma, A/B from 128B-swizzled SMEM (TMA), D in TMEM
@@ -25,12 +26,10 @@
 //   O_m[128x128] += P[128 x 128] . V_j       tcgen05.mma, A = P from TMEM, B = V (MN-major SMEM)
 //
 // TMEM (512 columns): O_0, O_1 (128 fp32 columns each), S_0/P_0, S_1/P_1 (128 each).
-// Warp roles (384 threads): warps 0..3 = softmax team 0, warps 4..7 = team 1, warp 8 = TMA producer,
-// warps 9 / 10 = MMA issuers of slot 0 / 1 (one thread each; warp 10 also owns the TMEM allocation),
-// warp 11 = zeroes the V rows behind a
+// Warp roles (384 threads): warps 0..7 = softmax (warps 0..3 key columns 0..63, warps 4..7 columns
+// 64..127 of every S tile), warp 8 = TMA producer, warps 9 / 10 = MMA issuers of slot 0 / 1 (one
+// thread each; warp 10 also owns the TMEM allocation), warp 11 = zeroes the V rows behind a
 // ragged tile end (they are multiplied by exact zeros and may hold anything, NaN included).  The
-// control warps have the HIGHEST warp ids on purpose: the SM's issue arbiter prefers higher warp ids,
-// and a starved MMA issuer stalls the whole pipeline while the softmax warps always have work.  The
 // control warpgroup gives registers to the softmax warpgroups (setmaxnreg).  The running max is only
 // raised when a tile maximum exceeds it by more than 2^8 (lazy rescale), in which case the owning
 // thread rescales its O row in TMEM before the next P.V.
@@ -63,8 +62,9 @@ constexpr uint32_t kKvTileBytes = kTileN * kD * 2;  // 32 KiB: [d_hi 2][128 keys
 constexpr uint32_t kOffQ = 0;
 constexpr uint32_t kOffRing = 2 * kQTileBytes;
 constexpr uint32_t kOffBar = kOffRing + kRing * kKvTileBytes;
-constexpr uint32_t kSmemUsed = kOffBar + 256;
-constexpr uint32_t kSmemBytes = kSmemUsed + 1024;         // + alignment slack (1024 B swizzle atoms)
+constexpr uint32_t kOffX = kOffBar + 256;                 // softmax exchange: fp32 [2][2][128]
+constexpr uint32_t kSmemUsed = kOffX + 2 * 2 * kTileM * 4;
+constexpr uint32_t kSmemBytes = 232448;                   // the whole 227 KiB: kSmemUsed + alignment slack
 constexpr uint32_t kTmemCols = 512;
 constexpr uint32_t kTmemS = 256;  // S/P buffers of the two slots behind the two O accumulators
 constexpr float kLog2e = 1.4426950408889634f;
@@ -82,11 +82,12 @@ enum : uint32_t {
     kBarAllDone = kBarPFull + 8,       // every MMA of the CTA has completed
     kBarVFix = kBarAllDone + 1,        // [2] warp 11 has zeroed the V rows behind a ragged tile end; a CTA
                                        // meets at most two ragged tiles (last prefix tile, last tree tile)
-    kNumBars = kBarVFix + 2,
+    kBarMerge = kBarVFix + 2,          // the group's partial O rows of this CTA's share have landed in shared memory
+    kNumBars = kBarMerge + 1,
     kTmemSlot = kNumBars  // uint32 written by tcgen05.alloc
 };
 static_assert((kNumBars + 1) * 8 <= 256, "barrier area");
-static_assert(kSmemBytes <= 232448, "shared memory budget");
+static_assert(kSmemUsed + 512 <= kSmemBytes, "shared memory budget");
 
 // ---- PTX wrappers -------------------------------------------------------------------------------
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
@@ -303,7 +304,9 @@ __device__ long long g_timeline[256][128];
     } while (0)
 // accumulate the cycles since the previous TLA of this thread into bucket `b` (dumped at slots 3..15)
 #define TLA(b) do { const long long _t = clock64(); tl_acc[(b)] += _t - tl_last; tl_last = _t; } while (0)
+#define TLABS(slot) do { if (warp == 0 && lane == 0) { const int _c = blockIdx.x + gridDim.x * blockIdx.y; if (_c < 256) g_timeline[_c][(slot)] = clock64(); } } while (0)
 #else
+#define TLABS(slot) do {} while (0)
 #define TL(slot) do {} while (0)
 #define TLA(b) do {} while (0)
 #endif
@@ -342,76 +345,104 @@ struct TileInfo {
 // -------------------------------------------------------------------------------------------------
 // Cascade merge of one group's rows (log-sum-exp state merge):
 //   LSE = log sum_p e^{LSE_p};  O = sum_p e^{LSE_p - LSE} O_p   over the partial states that hold the row.
-// Warp `gw` of `n_gw` takes rows gw, gw + n_gw, ... of the item.  A pair item has one state per chunk
-// (at partial rows c*256 + row), a split item two per chunk (at (2c+s)*128 + row).  Lane i first
-// fetches the LSE of state i, then the warp sweeps the states' O rows (512 B each, stored with their
-// 16-byte chunks XOR-swizzled by the row, undone here), eight loads in flight per lane.  The
-// partial states were written by other SMs: read them at L2 (ld.global.cg).
+// CTA `ci` of the group's `nc` CTAs takes a contiguous range of the item's rows.  A pair item has one
+// state per chunk (at partial rows c*256 + row), a split item two per chunk (at (2c+s)*128 + row).
+// One bulk copy per state brings the range's O rows (512 B each, stored with their 16-byte chunks
+// XOR-swizzled by the row, undone here) into shared memory -- all copies in flight at once, one L2
+// round trip -- while the LSEs are staged with plain loads.  Warp w then
+// merges rows w, w+8, ... of the range.  The partial states were written by other SMs through the
+// async proxy and published with a release; they are read at L2 (bulk copy / ld.global.cg).
 __device__ __forceinline__ void merge_rows(const AttnPlan& pl, const AttnArgs& a, float* dbg_rows, const Work& wk,
-                                           int gw, int n_gw, int lane) {
+                                           uint32_t smem_stage, unsigned char* stage_gen, uint32_t bar_merge,
+                                           int warp, int lane) {
     const int G = pl.G;
     const bool split = wk.mode == kModeSplit;
     const int rows_item = split ? wk.rows0 : wk.rows0 + wk.rows1;
-    const int n_rel = split ? 2 * wk.n_chunks : wk.n_chunks;
+    const int n_rel = split ? 2 * wk.n_chunks : wk.n_chunks;  // <= 128 states
     const size_t grp0 = (size_t)wk.group * pl.grp_rows;
-    for (int rr = gw; rr < rows_item; rr += n_gw) {
-        auto row_of = [&](int i) { return grp0 + (size_t)(split ? i * kTileM : i * 2 * kTileM) + rr; };
-        float m = -INFINITY, wsum = 0.f;
-        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-        for (int base = 0; base < n_rel; base += 32) {
-            const int i = base + lane;
-            const float l = i < n_rel ? __ldcg(a.part_lse + row_of(i)) : -INFINITY;
-            float mb = l;
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) mb = fmaxf(mb, __shfl_xor_sync(0xffffffffu, mb, o));
-            if (mb == -INFINITY) continue;
-            if (mb > m) {  // rescale what has been accumulated so far (only with > 32 states)
-                const float sc = m == -INFINITY ? 0.f : __expf(m - mb);
-                acc.x *= sc; acc.y *= sc; acc.z *= sc; acc.w *= sc;
-                wsum *= sc;
-                m = mb;
-            }
-            const float wl = l == -INFINITY ? 0.f : __expf(l - m);
-            const int cnt = min(32, n_rel - base);
-            for (int q0 = 0; q0 < cnt; q0 += 8) {
-                float4 o[8];
-                float w[8];
-#pragma unroll
-                for (int q = 0; q < 8; ++q) {
-                    w[q] = __shfl_sync(0xffffffffu, wl, (q0 + q) & 31);
-                    if (q0 + q >= cnt) w[q] = 0.f;
-                    o[q] = make_float4(0.f, 0.f, 0.f, 0.f);
-                    if (w[q] != 0.f)
-                        o[q] = __ldcg(reinterpret_cast<const float4*>(a.part_o + row_of(base + q0 + q) * kD) + lane);
-                }
-#pragma unroll
-                for (int q = 0; q < 8; ++q) {
-                    wsum += w[q];
-                    acc.x += w[q] * o[q].x; acc.y += w[q] * o[q].y; acc.z += w[q] * o[q].z; acc.w += w[q] * o[q].w;
-                }
-            }
+    const int stride = split ? kTileM : 2 * kTileM;
+    const int r0 = rows_item * wk.chunk / wk.n_chunks, r1 = rows_item * (wk.chunk + 1) / wk.n_chunks;
+    const int nrows = r1 - r0;  // nrows * n_rel <= 320 rows of 512 B: fits the freed Q + ring area
+    if (nrows <= 0) return;
+    if (warp == 0) {
+        if (lane == 0) mbar_expect_tx(bar_merge, (uint32_t)(n_rel * nrows) * 512u);
+        __syncwarp();
+        for (int i = lane; i < n_rel; i += 32)
+            asm volatile(
+                "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                    smem_stage + (uint32_t)(i * nrows) * 512u),
+                "l"(a.part_o + (grp0 + (size_t)i * stride + r0) * kD), "r"((uint32_t)nrows * 512u), "r"(bar_merge)
+                : "memory");
+    }
+    // the LSEs of the range's rows, all states, into shared memory behind the O block (one round trip)
+    float* lse_sm = reinterpret_cast<float*>(stage_gen + 320u * 512u);
+    const int tid = warp * 32 + lane;
+    for (int e = tid; e < n_rel * nrows; e += 256) {
+        const int i = e / nrows, r = e - i * nrows;
+        const float v = __ldcg(a.part_lse + grp0 + (size_t)i * stride + r0 + r);
+        lse_sm[e] = v;
+    }
+    named_bar_sync(1, 256);
+    TLABS(110);
+    auto out_row = [&](int r) {  // index of query row r0 + r of the item in out / lse: [b][t][h]
+        const int ra = wk.row_base + r0 + r, t = ra / G;
+        return ((size_t)wk.b * pl.T_cap + t) * pl.Hq + wk.g * G + (ra - t * G);
+    };
+    // step 1, one thread per row: LSE = m + log sum_p e^{LSE_p - m}; the LSEs in shared memory are
+    // replaced by the normalised weights e^{LSE_p - LSE} (a state without any key: weight 0)
+    if (tid < nrows) {
+        float* col0 = lse_sm + tid;
+        float m = -INFINITY;
+#pragma unroll 4
+        for (int i = 0; i < n_rel; ++i) m = fmaxf(m, col0[i * nrows]);
+        float wsum = 0.f;
+#pragma unroll 4
+        for (int i = 0; i < n_rel; ++i) {
+            const float v = col0[i * nrows];
+            const float wv = v == -INFINITY ? 0.f : __expf(v - m);
+            wsum += wv;
+            col0[i * nrows] = wv;
         }
         const float inv = wsum > 0.f ? 1.f / wsum : 0.f;  // no key at all (L = 0, prefix-only mode): O = 0, LSE = -inf
+#pragma unroll 4
+        for (int i = 0; i < n_rel; ++i) col0[i * nrows] *= inv;
         const float lse = wsum > 0.f ? m + logf(wsum) : -INFINITY;
-        const int r = wk.row_base + rr;
-        const int t = r / G;
-        const size_t orow = ((size_t)wk.b * pl.T_cap + t) * pl.Hq + wk.g * G + (r - t * G);
-        const int col = 4 * (lane ^ (rr & 7));  // undo the staging swizzle: this lane holds columns col..col+3
-        if (dbg_rows) {  // fp32 state for tests: d values of O, then the LSE
+        const size_t orow = out_row(tid);
+        if (dbg_rows) dbg_rows[orow * (kD + 1) + kD] = lse;
+        else if (a.lse) a.lse[orow] = lse;
+    }
+    named_bar_sync(1, 256);
+    mbar_wait(bar_merge, 0);  // the O rows have landed
+    TLABS(111);
+    // step 2, one thread per (row, 16-byte chunk): O = sum_p weight_p O_p.  States without any key hold
+    // zeros (their CTA wrote them), so no value needs guarding.
+#pragma unroll 1
+    for (int item = tid; item < nrows * 32; item += 256) {
+        const int r = item >> 5;  // == warp-uniform row; chunk position == lane
+        const float4* o_ptr = reinterpret_cast<const float4*>(stage_gen + (size_t)r * 512u) + lane;
+        const float* w_ptr = lse_sm + r;
+        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll 4
+        for (int i = 0; i < n_rel; ++i) {
+            const float wv = w_ptr[i * nrows];
+            const float4 o = o_ptr[(size_t)(i * nrows) * 32];
+            acc.x += wv * o.x; acc.y += wv * o.y; acc.z += wv * o.z; acc.w += wv * o.w;
+        }
+        const size_t orow = out_row(r);
+        const int col = 4 * (lane ^ ((r0 + r) & 7));  // undo the staging swizzle: this lane holds columns col..col+3
+        if (dbg_rows) {  // fp32 state for tests
             float* d0 = dbg_rows + orow * (kD + 1);
-            d0[col + 0] = acc.x * inv; d0[col + 1] = acc.y * inv;
-            d0[col + 2] = acc.z * inv; d0[col + 3] = acc.w * inv;
-            if (lane == 0) d0[kD] = lse;
+            d0[col + 0] = acc.x; d0[col + 1] = acc.y; d0[col + 2] = acc.z; d0[col + 3] = acc.w;
             continue;
         }
-        __nv_bfloat162 lo = __floats2bfloat162_rn(acc.x * inv, acc.y * inv);
-        __nv_bfloat162 hi = __floats2bfloat162_rn(acc.z * inv, acc.w * inv);
+        __nv_bfloat162 lo = __floats2bfloat162_rn(acc.x, acc.y);
+        __nv_bfloat162 hi = __floats2bfloat162_rn(acc.z, acc.w);
         uint2 pk;
         pk.x = *reinterpret_cast<uint32_t*>(&lo);
         pk.y = *reinterpret_cast<uint32_t*>(&hi);
         *reinterpret_cast<uint2*>(a.out + orow * kD + col) = pk;
-        if (a.lse && lane == 0) a.lse[orow] = lse;
     }
+    TLABS(113);
 }
 
 // mode bits: 1 = include the prefix tiles, 2 = include the tree tiles (3 = the whole cascade).
@@ -445,6 +476,7 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
         mbar_init(bar(kBarAllDone), 2);
         mbar_init(bar(kBarVFix + 0), 1);
         mbar_init(bar(kBarVFix + 1), 1);
+        mbar_init(bar(kBarMerge), 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         tma_prefetch_desc(&tm_q);
         tma_prefetch_desc(&tm_k);
@@ -519,6 +551,9 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
     if (tid == 0) TL(0);
+#ifdef D2SD_TIMELINE
+    if (tid == 0) g_timeline[blockIdx.x + gridDim.x * blockIdx.y][123] = tl_t0;
+#endif
 
     // the control warpgroup hands registers to the two softmax warpgroups (one instruction per warpgroup)
     if (warp >= 8) {
@@ -654,6 +689,8 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 if (n < 8) TL(16 + 6 * n + 3 * s + 2);
                 ++n;
 #endif
+                tc_commit(bar(kBarEmpty + vi));  // V_j is free once these P.V pieces have completed
+                TLA(4);
                 if (!next_ready) advance(true);
                 TLA(5);
 #ifdef D2SD_TIMELINE
@@ -661,8 +698,6 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
 #endif
                 if (nj < wk.n_tiles) issue_qk(nj, nki);
                 TLA(6);  // Q.K^T issue
-                tc_commit(bar(kBarEmpty + vi));
-                TLA(4);
                 jj = nj; ki = nki; kpar = nkpar;
             }
             tc_commit(bar(kBarAllDone));
@@ -709,83 +744,91 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
     } else {
       asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegsSoftmax));
       if (!idle) {
-        // ===== softmax team s (warps 4s .. 4s+3) serves slot s; thread (w, lane) owns query row
-        // w*32 + lane of the slot's tile (TMEM lane) and all 128 key columns of every S tile. =====
-        const int s = warp >> 2;
+        // ===== softmax: all eight warps serve ONE unit at a time, two threads per query row: warps 0..3
+        // take key columns 0..63 of the S tile, warps 4..7 columns 64..127; thread (w, lane) of either
+        // half owns query row w*32 + lane (TMEM lane).  Two warps per scheduler keep the MUFU pipe
+        // saturated (a single warp reaches only ~2/3 of it), and because the units alternate between
+        // the two slots, the tensor phase of one slot (P.V, next Q.K^T) runs under the other slot's
+        // softmax.  The halves exchange their row maxima through shared memory once per unit. =====
+        const int h = warp >> 2;
         const int w = warp & 3;
         const int rl = w * 32 + lane;  // row within the tile
         const uint32_t lane_addr = (uint32_t)(w * 32) << 16;
         const float c2 = pl.sm_scale * kLog2e;
         const float thr = kRescaleThreshold / c2;  // in raw score units
-        const bool slot_used = wk.mode != kModeSolo || s == 0;
-        const int rows_s = wk.rows(s);
+        float* xm = reinterpret_cast<float*>(smem_gen + kOffX);  // [2 unit parity][2 halves][128 rows]
+        // per-slot running state in scalars (selected by the unrolled s)
+        float m_run0 = -INFINITY, m_run1 = -INFINITY, l_run0 = 0.f, l_run1 = 0.f;
+        int kcnt0 = 0, kcnt1 = 0;
+        int n = 0;
+        for (int jj = 0; jj < wk.n_tiles; ++jj) {
+            const uint32_t use = wk.uses(jj);
+            const TileInfo ti = tile_info(jj);
+            const bool masked_tile = ti.tree || ti.valid < kTileN;
+#pragma unroll
+            for (int s = 0; s < 2; ++s) {
+                if (!((use >> s) & 1u)) continue;
+                const int k = s ? kcnt1 : kcnt0;
+                float m_cur = s ? m_run1 : m_run0, l_cur = s ? l_run1 : l_run0;
 #ifdef D2SD_DBG_NOSOFTMAX
-        const bool warp_active = false;  // timing experiment only: results are garbage
+                const bool warp_active = false;  // timing experiment only: results are garbage
 #else
-        const bool warp_active = slot_used && w * 32 < rows_s;
+                const bool warp_active = w * 32 < wk.rows(s);
 #endif
-        const uint32_t sbuf = tmem + kTmemS + s * kTileN + lane_addr;
-        const uint32_t o_addr = tmem + s * kD + lane_addr;
-        float m_run = -INFINITY, l_run = 0.f;
-        int k = 0;  // units of this slot so far
-        // The exponentials of a unit saturate the SM's MUFU pipe, so the two teams take turns at them
-        // (named barriers 2 / 3, one hands the turn to the other): team 0's exp phase then overlaps team
-        // 1's tensor phase and vice versa instead of both teams computing and both waiting in step.
-        const bool pingpong = wk.mode != kModeSolo;
-        if (pingpong && s == 1) named_bar_arrive(2, 256);  // team 0 goes first
-        if (slot_used) {
-            for (int jj = 0; jj < wk.n_tiles; ++jj) {
-                if (!((wk.uses(jj) >> s) & 1u)) continue;
-                const TileInfo ti = tile_info(jj);
-                const bool masked_tile = ti.tree || ti.valid < kTileN;
+                const uint32_t sbuf = tmem + kTmemS + s * kTileN + lane_addr;
+                const uint32_t o_addr = tmem + s * kD + h * 64 + lane_addr;
                 mbar_wait(bar(kBarSFull + s), k & 1);
-                if (w == 0 && lane == 0 && k < 8) TL(64 + 4 * k + 2 * s);
-                uint32_t sv[128];
-                float ms = 0.f;
+                if (warp == 0 && lane == 0 && n < 16) TL(64 + 2 * n);
+                uint32_t sv[64];
+                float mxh = -INFINITY;
                 if (warp_active) {
                     tc_fence_after();
-                    D2SD_TMEM_LD32(sbuf, sv, 0);
-                    D2SD_TMEM_LD32(sbuf + 32, sv, 32);
-                    D2SD_TMEM_LD32(sbuf + 64, sv, 64);
-                    D2SD_TMEM_LD32(sbuf + 96, sv, 96);
+                    D2SD_TMEM_LD32(sbuf + h * 64, sv, 0);
+                    D2SD_TMEM_LD32(sbuf + h * 64 + 32, sv, 32);
                     tmem_wait_ld();
-                    if (w == 0 && lane == 0 && k == 3) TL(102 + 8 * s);
                     if (masked_tile) {
                         // keys past the tile's end, and (tree tiles) keys that are not ancestors-or-self of
-                        // this row's node: the tile's 128 mask bits -> -inf
-                        uint32_t mw[4] = {0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu};
+                        // this row's node: bits 64h..64h+63 of the tile's 128 mask bits, -> -inf
+                        uint32_t mw0 = 0xFFFFFFFFu, mw1 = 0xFFFFFFFFu;
                         if (ti.tree) {
                             const int t = min((wk.row_base + wk.row_off(s) + rl) / pl.G, wk.T - 1);
                             const uint32_t* mrow = a.mask + ((size_t)wk.b * pl.T_cap + t) * pl.W;
-#pragma unroll
-                            for (int q = 0; q < 4; ++q) mw[q] = ti.tt * 4 + q < pl.W ? mrow[ti.tt * 4 + q] : 0u;
+                            const int wi = ti.tt * 4 + h * 2;
+                            mw0 = wi < pl.W ? mrow[wi] : 0u;
+                            mw1 = wi + 1 < pl.W ? mrow[wi + 1] : 0u;
                         }
+                        const int lim = ti.valid - h * 64;  // columns [lim, 64) of this half are past the end
 #pragma unroll
-                        for (int c = 0; c < 128; ++c) {
-                            const uint32_t bit = (mw[c >> 5] >> (c & 31)) & 1u;
-                            if (c >= ti.valid || !bit) sv[c] = 0xFF800000u;
+                        for (int c = 0; c < 64; ++c) {
+                            const uint32_t bit = ((c < 32 ? mw0 : mw1) >> (c & 31)) & 1u;
+                            if (c >= lim || !bit) sv[c] = 0xFF800000u;
                         }
                     }
                     float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;
 #pragma unroll
-                    for (int c = 0; c < 128; c += 4) {
+                    for (int c = 0; c < 64; c += 4) {
                         mx0 = fmaxf(mx0, __uint_as_float(sv[c]));
                         mx1 = fmaxf(mx1, __uint_as_float(sv[c + 1]));
                         mx2 = fmaxf(mx2, __uint_as_float(sv[c + 2]));
                         mx3 = fmaxf(mx3, __uint_as_float(sv[c + 3]));
                     }
-                    const float mx = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
+                    mxh = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
+                }
+                xm[((n & 1) * 2 + h) * kTileM + rl] = mxh;
+                named_bar_sync(1, 256);  // also orders "both halves have read S" before "P overwrites S"
+                if (warp_active) {
+                    const float mx = fmaxf(mxh, xm[((n & 1) * 2 + (h ^ 1)) * kTileM + rl]);
                     // lazy rescale: raise the running max only when it is exceeded by more than 2^8
-                    const bool need = mx > m_run + thr;
+                    const bool need = mx > m_cur + thr;
                     if (k == 0) {
-                        m_run = mx;
+                        m_cur = mx;
                     } else if (__any_sync(0xffffffffu, need)) {
-                        const float alpha = need ? ex2((m_run - mx) * c2) : 1.f;
+                        const float alpha = need ? ex2((m_cur - mx) * c2) : 1.f;
                         // S_k ready implies the previous P.V into this O has landed (tcgen05.commit covers
                         // every earlier MMA of the issuing thread)
                         tc_fence_after();
 #pragma unroll 1
-                        for (int c0 = 0; c0 < kD; c0 += 32) {
+                        for (int c0 = 0; c0 < 64; c0 += 32) {  // this half's 64 of the 128 O columns
                             uint32_t o[32];
                             D2SD_TMEM_LD32(o_addr + c0, o, 0);
                             tmem_wait_ld();
@@ -795,30 +838,25 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                         }
                         tmem_wait_st();
                         if (need) {
-                            m_run = mx;
-                            l_run *= alpha;
+                            m_cur = mx;
+                            l_cur *= alpha;
                         }
                     }
                     // a row with every key so far masked has m_run = -inf: exp2(-inf - 0) = 0, not NaN
-                    ms = m_run == -INFINITY ? 0.f : m_run * c2;
-                    if (w == 0 && lane == 0 && k == 3) TL(103 + 8 * s);
-                }
-                if (pingpong) named_bar_sync(2 + s, 256);  // this team's turn at the exponentials
-                if (w == 0 && lane == 0 && k == 3) TL(104 + 8 * s);
-                if (warp_active) {
+                    const float ms = m_cur == -INFINITY ? 0.f : m_cur * c2;
                     float sum0 = 0.f, sum1 = 0.f;
-                    // P[128 x 128] bf16 = 64 TMEM columns, released 16 at a time.  The store of piece q is
-                    // only waited for after the exponentials of piece q+1 have been issued, so the MUFU
-                    // pipe never idles behind a TMEM store.
+                    // P[128 x 128] bf16 = 64 TMEM columns; this half writes columns 32h..32h+31 in two
+                    // pieces (key quarters 2h, 2h+1), each released to the tensor pipe on its own.  The
+                    // store of a piece is only waited for after the next piece's exponentials.
 #pragma unroll
-                    for (int q = 0; q < 4; ++q) {
+                    for (int q = 0; q < 2; ++q) {
                         float ev[32];
 #pragma unroll
                         for (int c = 0; c < 32; ++c) ev[c] = ex2_ordered(__uint_as_float(sv[q * 32 + c]) * c2 - ms);
-                        if (q > 0) {  // piece q-1 has landed in TMEM long ago: release it
+                        if (q > 0) {
                             tmem_wait_st();
                             tc_fence_before();
-                            mbar_arrive(bar(kBarPFull + 4 * s + q - 1));
+                            mbar_arrive(bar(kBarPFull + 4 * s + 2 * h));
                         }
                         uint32_t p[16];
                         float t0 = 0.f, t1 = 0.f, t2 = 0.f, t3 = 0.f;
@@ -830,47 +868,59 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                         }
                         sum0 += t0 + t1;
                         sum1 += t2 + t3;
-                        D2SD_TMEM_ST16(sbuf + q * 16, p);
+                        D2SD_TMEM_ST16(sbuf + h * 32 + q * 16, p);
                     }
-                    if (w == 0 && lane == 0 && k == 3) TL(105 + 8 * s);
-                    if (pingpong) named_bar_arrive(3 - s, 256);  // exponentials issued: hand the turn over
-                    l_run += sum0 + sum1;
+                    l_cur += sum0 + sum1;
                     tmem_wait_st();
                     tc_fence_before();
-                    mbar_arrive(bar(kBarPFull + 4 * s + 3));
+                    mbar_arrive(bar(kBarPFull + 4 * s + 2 * h + 1));
                 } else {
-#pragma unroll
-                    for (int q = 0; q < 4; ++q) mbar_arrive(bar(kBarPFull + 4 * s + q));
-                    if (pingpong) named_bar_arrive(3 - s, 256);
+                    mbar_arrive(bar(kBarPFull + 4 * s + 2 * h));
+                    mbar_arrive(bar(kBarPFull + 4 * s + 2 * h + 1));
                 }
-                if (w == 0 && lane == 0 && k < 8) TL(64 + 4 * k + 2 * s + 1);
-                ++k;
+                if (warp == 0 && lane == 0 && n < 16) TL(64 + 2 * n + 1);
+                if (s) { m_run1 = m_cur; l_run1 = l_cur; ++kcnt1; } else { m_run0 = m_cur; l_run0 = l_cur; ++kcnt0; }
+                ++n;
             }
         }
         // ---- epilogue: O / l -> swizzled staging image in shared memory -> bulk copies to the slot's
         // partial state (row r of the image: 32 chunks of 16 B, chunk c stored at position c ^ (r & 7)) ----
         mbar_wait(bar(kBarAllDone), 0);  // every MMA done: the ring is free for staging
-        if (w == 0 && lane == 0) TL(100 + 8 * s);
-        if (slot_used) {
+        if (warp == 0 && lane == 0) TL(100);
+#pragma unroll 1
+        for (int s = 0; s < 2; ++s) {
+            if (wk.mode == kModeSolo && s == 1) continue;
+            const float m_fin = s ? m_run1 : m_run0, l_fin = s ? l_run1 : l_run0;
+            const int rows_s = wk.rows(s);
             const size_t prow0 = (size_t)wk.group * pl.grp_rows + wk.part_row0(s);
             float* po = a.part_o + prow0 * kD;
             float* plse = a.part_lse + prow0;
             const bool row_ok = rl < rows_s;
-            if (k == 0) {  // no unit for this slot (empty chunk 0, or a split chunk of a single key tile)
-                if (row_ok) plse[rl] = -INFINITY;
-            } else if (warp_active) {
+            if ((s ? kcnt1 : kcnt0) == 0) {  // no unit for this slot (empty chunk 0, or a split chunk of a single key tile)
+                if (h == 0 && row_ok) plse[rl] = -INFINITY;
+                if (row_ok)  // the merge reads every state's O unguarded: give it zeros (weight 0 anyway)
+                    for (int c = h * 16; c < h * 16 + 16; ++c)
+                        reinterpret_cast<float4*>(po + (size_t)rl * kD)[c] = make_float4(0.f, 0.f, 0.f, 0.f);
+                continue;
+            }
+            const bool warp_active = w * 32 < rows_s;
+            xm[h * kTileM + rl] = l_fin;
+            named_bar_sync(1, 256);
+            const float l_tot = l_fin + xm[(h ^ 1) * kTileM + rl];
+            const uint32_t stage = smem + kOffRing + (uint32_t)s * (2 * kKvTileBytes);
+            if (warp_active) {
                 tc_fence_after();
-                const float inv = l_run > 0.f ? 1.f / l_run : 0.f;  // l = 0: every key of the chunk masked
-                const uint32_t stage = smem + kOffRing + (uint32_t)s * (2 * kKvTileBytes);
+                const float inv = l_tot > 0.f ? 1.f / l_tot : 0.f;  // l = 0: every key of the chunk masked
                 const uint32_t srow = stage + (uint32_t)rl * 512u;
+                const uint32_t o_addr = tmem + s * kD + h * 64 + lane_addr;
 #pragma unroll
-                for (int c0 = 0; c0 < kD; c0 += 32) {
+                for (int c0 = 0; c0 < 64; c0 += 32) {
                     uint32_t o[32];
                     D2SD_TMEM_LD32(o_addr + c0, o, 0);
                     tmem_wait_ld();
 #pragma unroll
                     for (int c = 0; c < 32; c += 4) {
-                        const uint32_t chunk = (uint32_t)((c0 + c) >> 2);
+                        const uint32_t chunk = (uint32_t)((h * 64 + c0 + c) >> 2);
                         const uint32_t phys = chunk ^ ((uint32_t)rl & 7u);
                         asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(srow + phys * 16u),
                                      "f"(__uint_as_float(o[c]) * inv), "f"(__uint_as_float(o[c + 1]) * inv),
@@ -878,43 +928,48 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                                      : "memory");
                     }
                 }
-                if (row_ok) plse[rl] = l_run > 0.f ? m_run * pl.sm_scale + logf(l_run) : -INFINITY;
+                if (h == 0 && row_ok) plse[rl] = l_tot > 0.f ? m_fin * pl.sm_scale + logf(l_tot) : -INFINITY;
                 fence_async_smem();
-                __syncwarp();
-                if (lane == 0) {  // this warp's rows: one contiguous piece of the image and of the partial state
-                    const int nrows = min(32, rows_s - w * 32);
-                    bulk_store(po + (size_t)(w * 32) * kD, stage + (uint32_t)(w * 32) * 512u, (uint32_t)nrows * 512u);
-                    bulk_commit();
-                    bulk_wait_all();
-                    asm volatile("fence.proxy.async;" ::: "memory");
-                }
-                __syncwarp();
+            }
+            named_bar_sync(1, 256);  // both halves of every row are staged
+            if (warp_active && h == (s & 1) && lane == 0) {
+                // this warp's rows: one contiguous piece of the image and of the partial state
+                const int nrows = min(32, rows_s - w * 32);
+                bulk_store(po + (size_t)(w * 32) * kD, stage + (uint32_t)(w * 32) * 512u, (uint32_t)nrows * 512u);
+                bulk_commit();
             }
         }
-        if (w == 0 && lane == 0) TL(101 + 8 * s);
+        if (lane == 0) {
+            bulk_wait_all();
+            asm volatile("fence.proxy.async;" ::: "memory");
+        }
+        __syncwarp();
+        if (warp == 0 && lane == 0) TL(101);
 
         // ---- publish this CTA's partial states, wait for the group, merge this CTA's share of rows ----
         const unsigned expected = (unsigned)wk.n_chunks;
         unsigned* cnt = a.counters + 2 * wk.group;  // [0] arrivals, [1] done
-        __threadfence();
-        named_bar_sync(1, 256);
+        named_bar_sync(1, 256);  // every thread's partial-state writes happen before the leader's release
+        unsigned done_before = 0;
         if (warp == 0 && lane == 0) {
             asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(cnt) : "memory");
             unsigned seen, spins = 0;
             do {
                 asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(cnt) : "memory");
                 if (seen < expected) {
-                    __nanosleep(32);
+                    __nanosleep(20);
                     if (++spins > (1u << 24)) __trap();  // a scheduling assumption broke: fail, do not hang
                 }
             } while (seen < expected);
+            // this CTA is past the wait: count it out now, the round trip hides behind the merge
+            done_before = atomicAdd(cnt + 1, 1u);
         }
         named_bar_sync(1, 256);
         if (warp == 0 && lane == 0) TL(120);
-        merge_rows(pl, a, dbg_rows, wk, wk.chunk * 8 + warp, wk.n_chunks * 8, lane);
-        named_bar_sync(1, 256);
+        asm volatile("fence.proxy.async;" ::: "memory");  // the bulk copies below read what the acquire made visible
+        merge_rows(pl, a, dbg_rows, wk, smem + kOffQ, smem_gen + kOffQ, bar(kBarMerge), warp, lane);
         if (warp == 0 && lane == 0) {
-            if (atomicAdd(cnt + 1, 1u) == expected - 1) {  // last CTA out: everybody is past the wait
+            if (done_before == expected - 1) {  // last CTA out: everybody is past the wait
                 cnt[0] = 0;
                 cnt[1] = 0;
             }
