@@ -258,13 +258,13 @@ class Workload:
 
     @property
     def attn_kernel(self) -> str:
-        return "attn_mma_kernel" if self.cfg.paged else "attn_cascade_tc_kernel"
+        return "attn_cascade_tc_kernel"
 
     @property
     def launches_per_step(self) -> int:
         # select, build, per layer: one fused tcgen05 launch (contiguous KV) or mma.sync pass + merge
         # (paged KV), argmax, walk
-        return 2 + (2 if self.cfg.paged else 1) * self.cfg.layers + 2
+        return 2 + self.cfg.layers + 2
 
     # --- e2e: host buffers in, host results out ---------------------------------------------------
     def h2d_bytes(self, with_kv: bool) -> int:

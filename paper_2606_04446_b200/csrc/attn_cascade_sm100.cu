@@ -340,6 +340,7 @@ struct TileInfo {
     int row;        // first row of the tile in its tensor map
     bool tree;      // tree tile (ancestor mask applies), else prefix tile
     int tt;         // tree tile index (tree tiles only)
+    int j;          // key tile index within the request (prefix tiles first)
 };
 
 // -------------------------------------------------------------------------------------------------
@@ -539,10 +540,11 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
     auto tile_info = [&](int jj) {
         const int j = wk.j_begin + jj;
         TileInfo ti;
+        ti.j = j;
         ti.tree = j >= wk.np;
         ti.tt = j - wk.np;
         ti.valid = ti.tree ? min(kTileN, wk.T - ti.tt * kTileN) : min(kTileN, wk.L - j * kTileN);
-        ti.row = ti.tree ? wk.b * pl.T_cap + ti.tt * kTileN : kv_row0 + j * kTileN;
+        ti.row = ti.tree ? wk.b * pl.T_cap + ti.tt * kTileN : kv_row0 + j * kTileN;  // (contiguous KV)
         return ti;
     };
 
@@ -561,30 +563,58 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
       if (idle) {
         // fall through to the TMEM release
       } else if (warp == 8) {
-        // ===== TMA producer: K_0 first (the first MMA needs it), then the Q tiles, then the ring =====
-        if (elect_one()) {
-            int x = 0;  // ring position of the next tile to load
-            for (int jj = 0; jj < wk.n_tiles; ++jj) {
-                const TileInfo ti = tile_info(jj);
-                for (int kv = 0; kv < 2; ++kv, ++x) {
-                    const int i = x % kRing;
+        // ===== TMA producer: K_0 first (the first MMA needs it), then the Q tiles, then the ring.
+        // Contiguous KV: lane 0 issues one 32 KiB box per tile.  Paged KV (page = 16 keys): a 128-key
+        // tile is 8 pages; lane 2p+hi issues the 2 KiB box (page p, d half hi) of the tile, so a tile is
+        // 16 loads in flight at once.  Only the ceil(valid/16) pages that exist are loaded: the MMAs
+        // never read past ceil16(valid) keys.  The page ids of the next tile are fetched one tile ahead. =====
+        const bool paged = pl.page_size > 0;
+        int x = 0;  // ring position of the next tile to load
+        auto page_of = [&](int jj) {
+            int pg = 0;
+            if (paged && jj < wk.n_tiles) {
+                const TileInfo t2 = tile_info(jj);
+                const int p = lane >> 1;
+                if (!t2.tree && lane < 16 && p * 16 < t2.valid) pg = __ldg(a.kv_indices + kv_row0 + t2.j * 8 + p);
+            }
+            return pg;
+        };
+        int page_cur = page_of(0);
+        for (int jj = 0; jj < wk.n_tiles; ++jj) {
+            const TileInfo ti = tile_info(jj);
+            const int page_next = page_of(jj + 1);
+            for (int kv = 0; kv < 2; ++kv, ++x) {
+                const int i = x % kRing;
+                const uint32_t dst = smem + kOffRing + i * kKvTileBytes;
+                if (paged && !ti.tree) {
+                    const int n_pages = (ti.valid + 15) >> 4;
+                    if (lane == 0) {
+                        mbar_wait(bar(kBarEmpty + i), ((x / kRing) & 1) ^ 1);
+                        mbar_expect_tx(bar(kBarFull + i), (uint32_t)n_pages * 4096u);
+                    }
+                    __syncwarp();
+                    if (lane < 2 * n_pages)
+                        tma_load_5d(dst + (uint32_t)(lane & 1) * (kKvTileBytes / 2) + (uint32_t)(lane >> 1) * 2048u,
+                                    kv ? &tm_v : &tm_k, bar(kBarFull + i), 0, 0, lane & 1, wk.g, page_cur, kEvictFirst);
+                } else if (lane == 0) {
                     mbar_wait(bar(kBarEmpty + i), ((x / kRing) & 1) ^ 1);
                     mbar_expect_tx(bar(kBarFull + i), kKvTileBytes);
                     const CUtensorMap* tm = ti.tree ? (kv ? &tm_tv : &tm_tk) : (kv ? &tm_v : &tm_k);
-                    tma_load_4d(smem + kOffRing + i * kKvTileBytes, tm, bar(kBarFull + i), 0, ti.row, 0, wk.g,
-                                ti.tree ? kEvictLast : kEvictFirst);
-                    if (x == 0) {
-                        // a split item holds one M tile (Q buffer 0 serves both slots)
-                        const int nq = wk.mode == kModePair ? 2 : 1;
-                        for (int s = 0; s < nq; ++s) {
-                            const int t0 = wk.b * pl.T_cap + (wk.row_base + s * kTileM) / pl.G;
-                            mbar_expect_tx(bar(kBarQFull + s), kQTileBytes);
-                            tma_load_5d(smem + kOffQ + s * kQTileBytes, &tm_q, bar(kBarQFull + s), 0, 0, t0, 0, wk.g,
-                                        kEvictLast);
-                        }
+                    tma_load_4d(dst, tm, bar(kBarFull + i), 0, ti.row, 0, wk.g, ti.tree ? kEvictLast : kEvictFirst);
+                }
+                if (x == 0 && lane == 0) {
+                    // a split item holds one M tile (Q buffer 0 serves both slots)
+                    const int nq = wk.mode == kModePair ? 2 : 1;
+                    for (int s = 0; s < nq; ++s) {
+                        const int t0 = wk.b * pl.T_cap + (wk.row_base + s * kTileM) / pl.G;
+                        mbar_expect_tx(bar(kBarQFull + s), kQTileBytes);
+                        tma_load_5d(smem + kOffQ + s * kQTileBytes, &tm_q, bar(kBarQFull + s), 0, 0, t0, 0, wk.g,
+                                    kEvictLast);
                     }
                 }
+                __syncwarp();
             }
+            page_cur = page_next;
         }
       } else if (warp == 9 || warp == 10) {
         // ===== MMA issuers: one elected thread per SLOT (warp 9 -> slot 0, warp 10 -> slot 1).  The two
@@ -1018,9 +1048,9 @@ int32_t encode(CUtensorMap* tm, const void* base, int rank, const cuuint64_t* di
 }  // namespace
 
 bool attn_cascade_tc_supported(const AttnPlan& pl) {
-    // contiguous KV only (paged KV stays on the mma.sync path), rows of one query tile must be whole
-    // tree nodes (128 % G == 0), and the tensor-map extents must fit.
-    return pl.page_size == 0 && pl.d == kD && pl.G <= 128 && (128 % pl.G) == 0 &&
+    // contiguous or 16-key-paged KV, rows of one query tile must be whole tree nodes (128 % G == 0),
+    // and the tensor-map extents must fit.
+    return (pl.page_size == 0 || pl.page_size == 16) && pl.d == kD && pl.G <= 128 && (128 % pl.G) == 0 &&
            (int64_t)pl.B * pl.T_cap < (1ll << 31) && pl.kv_rows < (1ll << 31);
 }
 
@@ -1045,7 +1075,17 @@ int32_t launch_attn_cascade_tc(const AttnPlan& pl, const AttnArgs& a, int mode, 
         const cuuint64_t tdims[4] = {64, (cuuint64_t)pl.B * pl.T_cap, 2, (cuuint64_t)pl.Hkv};
         if (int32_t st = encode(&tm_tk, a.tree_k, 4, tdims, strides, box, "tree_k")) return st;
         if (int32_t st = encode(&tm_tv, a.tree_v, 4, tdims, strides, box, "tree_v")) return st;
-        if (pl.kv_rows > 0 && a.k_cache && a.v_cache) {
+        if (pl.kv_rows > 0 && a.k_cache && a.v_cache && pl.page_size > 0) {
+            // paged pool [P, 16, Hkv, d] viewed as (d_lo 64, slot 16, d_hi 2, g, page): one box = one d half
+            // of one page of one kv head (2 KiB); 16 boxes make a 128-key tile in the same shared-memory
+            // image as a contiguous tile (the 128B swizzle is a function of the shared-memory address)
+            const cuuint64_t pdims[5] = {64, 16, 2, (cuuint64_t)pl.Hkv, (cuuint64_t)(pl.kv_rows / 16)};
+            const cuuint64_t pstrides[4] = {(cuuint64_t)pl.Hkv * kD * 2, 128, (cuuint64_t)kD * 2,
+                                            (cuuint64_t)16 * pl.Hkv * kD * 2};
+            const cuuint32_t pbox[5] = {64, 16, 1, 1, 1};
+            if (int32_t st = encode(&tm_k, a.k_cache, 5, pdims, pstrides, pbox, "k_pool")) return st;
+            if (int32_t st = encode(&tm_v, a.v_cache, 5, pdims, pstrides, pbox, "v_pool")) return st;
+        } else if (pl.kv_rows > 0 && a.k_cache && a.v_cache) {
             const cuuint64_t dims[4] = {64, (cuuint64_t)pl.kv_rows, 2, (cuuint64_t)pl.Hkv};
             if (int32_t st = encode(&tm_k, a.k_cache, 4, dims, strides, box, "k_cache")) return st;
             if (int32_t st = encode(&tm_v, a.v_cache, 4, dims, strides, box, "v_cache")) return st;

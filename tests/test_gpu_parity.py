@@ -234,18 +234,22 @@ def test_attn_batched_contiguous_ragged(d2sd, oracle, impl):
     _attn_full_case(d2sd, oracle, cfg, impl=impl)
 
 
-def test_attn_tcgen05_is_the_default_for_contiguous_kv(d2sd):
-    """impl = 2 (force tcgen05) is accepted exactly where auto picks it; paged KV is not covered yet."""
+def test_attn_tcgen05_is_the_default(d2sd):
+    """impl = 2 (force tcgen05) is accepted exactly where auto picks it: contiguous and 16-key-paged KV
+    with 128 % G == 0; a GQA group size that does not divide a query tile stays on mma.sync."""
     assert d2sd.cascade_workspace_bytes(1, 70, 32, 8, 128, 4096, kv_rows=4096, impl=2) > 0
+    assert d2sd.cascade_workspace_bytes(1, 70, 32, 8, 128, 4096, page_size=16, kv_rows=8192, impl=2) > 0
     with pytest.raises(d2sd.D2sdError):
-        d2sd.cascade_workspace_bytes(1, 70, 32, 8, 128, 4096, page_size=16, kv_rows=8192, impl=2)
+        d2sd.cascade_workspace_bytes(1, 70, 24, 8, 128, 4096, kv_rows=4096, impl=2)
 
 
-def test_attn_paged_ragged_reduced_config5(d2sd, oracle):
+@pytest.mark.parametrize("impl", IMPLS)
+@pytest.mark.parametrize("ctx", [(1, 900), (0, 40), (2000, 2300)])
+def test_attn_paged_ragged_reduced_config5(d2sd, oracle, impl, ctx):
     """Config 5 at reduced size: paged KV (page 16, random page table, partial tail pages), ragged
     contexts; slots no request owns are NaN and must never reach an output."""
-    cfg = synth.custom(91, B=6, gamma=16, K=4, ctx=(1, 900), paged=True)
-    _attn_full_case(d2sd, oracle, cfg, pool_nan=True)
+    cfg = synth.custom(91, B=6, gamma=16, K=4, ctx=ctx, paged=True)
+    _attn_full_case(d2sd, oracle, cfg, pool_nan=True, impl=impl)
 
 
 @pytest.mark.parametrize("impl", IMPLS)
