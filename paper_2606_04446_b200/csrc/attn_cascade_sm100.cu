@@ -312,10 +312,11 @@ __device__ long long g_timeline[256][128];
 #endif
 
 // What one CTA does: which item / chunk, which rows its two slots hold, which key tiles it streams.
-enum : int { kModePair = 0, kModeSolo = 1, kModeSplit = 2 };
+enum : int { kModePair = 0, kModeSplit = 2 };
 struct Work {
     int b, g, item, chunk;
-    int mode;          // pair: both slots on every key tile; solo: slot 0 only; split: slot = key-tile parity
+    int mode;          // pair: both slots on every key tile; split: one query tile, slot = key-tile parity
+    int lay_pair;      // partial-state layout of the group: 1 = pair item (256 rows per chunk), 0 = 128 rows
     int row_base;      // first query row (t*G + hh) of the item
     int rows0, rows1;  // valid query rows of slot 0 / 1 (0 = slot unused)
     int np, nt;        // prefix / tree key tiles of the request (after the mode bits)
@@ -323,15 +324,16 @@ struct Work {
     int n_chunks;      // non-empty chunks of the group = CTAs that arrive at the group counter
     int group;         // (b*Hkv + g)*n_items + item
     int T, L, rows_valid;
+    int rows_item;     // valid query rows of the whole item (<= 256 for a pair item)
     __device__ __forceinline__ int rows(int s) const { return s ? rows1 : rows0; }
     // slot's first row relative to row_base (0 / 128 for a pair, 0 / 0 for a split)
     __device__ __forceinline__ int row_off(int s) const { return mode == kModeSplit ? 0 : s * kTileM; }
     __device__ __forceinline__ uint32_t uses(int jj) const {  // slots fed by the chunk's jj-th key tile
-        return mode == kModePair ? 3u : mode == kModeSolo ? 1u : (1u << (jj & 1));
+        return mode == kModePair ? 3u : (1u << (jj & 1));
     }
     // partial-state row of (slot s, row rl of the slot's tile) inside the group's partial block
     __device__ __forceinline__ int part_row0(int s) const {
-        return mode == kModeSplit ? (2 * chunk + s) * kTileM : chunk * 2 * kTileM + s * kTileM;
+        return lay_pair ? chunk * 2 * kTileM + s * kTileM : chunk * kTileM;
     }
 };
 
@@ -347,7 +349,7 @@ struct TileInfo {
 // Cascade merge of one group's rows (log-sum-exp state merge):
 //   LSE = log sum_p e^{LSE_p};  O = sum_p e^{LSE_p - LSE} O_p   over the partial states that hold the row.
 // CTA `ci` of the group's `nc` CTAs takes a contiguous range of the item's rows.  A pair item has one
-// state per chunk (at partial rows c*256 + row), a split item two per chunk (at (2c+s)*128 + row).
+// state per chunk and query tile (at partial rows c*256 + row), a split item one per chunk (at c*128 + row).
 // One bulk copy per state brings the range's O rows (512 B each, stored with their 16-byte chunks
 // XOR-swizzled by the row, undone here) into shared memory -- all copies in flight at once, one L2
 // round trip -- while the LSEs are staged with plain loads.  Warp w then
@@ -357,9 +359,9 @@ __device__ __forceinline__ void merge_rows(const AttnPlan& pl, const AttnArgs& a
                                            uint32_t smem_stage, unsigned char* stage_gen, uint32_t bar_merge,
                                            int warp, int lane) {
     const int G = pl.G;
-    const bool split = wk.mode == kModeSplit;
-    const int rows_item = split ? wk.rows0 : wk.rows0 + wk.rows1;
-    const int n_rel = split ? 2 * wk.n_chunks : wk.n_chunks;  // <= 128 states
+    const bool split = !wk.lay_pair;
+    const int rows_item = wk.rows_item;
+    const int n_rel = wk.n_chunks;  // <= 64 states
     const size_t grp0 = (size_t)wk.group * pl.grp_rows;
     const int stride = split ? kTileM : 2 * kTileM;
     const int r0 = rows_item * wk.chunk / wk.n_chunks, r1 = rows_item * (wk.chunk + 1) / wk.n_chunks;
@@ -515,16 +517,20 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
         wk.T = a.tree_len[wk.b];
         wk.L = a.ctx_len[wk.b];
         wk.rows_valid = wk.T * G;
-        wk.row_base = wk.item * 2 * kTileM;
+        wk.row_base = wk.item < pl.n_pair ? wk.item * 2 * kTileM
+                                          : (pl.n_pair * 2 + (wk.item - pl.n_pair)) * kTileM;
         wk.group = (wk.b * pl.Hkv + wk.g) * (pl.n_pair + pl.n_single) + wk.item;
         const int left = wk.rows_valid - wk.row_base;
         wk.rows0 = max(0, min(kTileM, left));
         if (wk.mode == kModePair) {
             wk.rows1 = max(0, min(kTileM, left - kTileM));
-            if (wk.rows1 == 0) wk.mode = kModeSolo;
-        } else {
-            wk.rows1 = wk.rows0;
+            // a pair item whose second query tile is empty (short tree): run the one tile as a split item
+            // (both slots, key-tile parity), keep the pair item's partial-state layout
+            if (wk.rows1 == 0) wk.mode = kModeSplit;
         }
+        wk.lay_pair = wk.item < pl.n_pair;
+        wk.rows_item = max(0, min(wk.lay_pair ? 2 * kTileM : kTileM, left));
+        if (wk.mode == kModeSplit) wk.rows1 = wk.rows0;
         wk.np = (mode & 1) ? (wk.L + kTileN - 1) / kTileN : 0;
         wk.nt = (mode & 2) ? (wk.T + kTileN - 1) / kTileN : 0;
         const int nk = wk.np + wk.nt;
@@ -626,7 +632,6 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
         // its fill has been observed (so the arrival can only count for that fill). =====
         if (elect_one()) {
             const int s = warp - 9;
-            const bool slot_used = wk.mode != kModeSolo || s == 0;
             const uint64_t qd = smem_desc(smem + kOffQ + (wk.mode == kModePair && s ? kQTileBytes : 0u), 16, 1024);
             const uint32_t sd = tmem + kTmemS + s * kTileN;  // S, overwritten by P (bf16, 64 columns)
             const uint32_t od = tmem + s * kD;
@@ -637,7 +642,7 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
 #endif
             int jj = 0, ki = 0, kpar = 0;  // current tile and the ring slot / fill parity of its K
             auto ring_next = [&](int& i, int& p) { if (++i == kRing) { i = 0; p ^= 1; } };
-            auto is_used = [&](int j) { return slot_used && ((wk.uses(j) >> s) & 1u); };
+            auto is_used = [&](int j) { return ((wk.uses(j) >> s) & 1u) != 0; };
             auto valid_of = [&](int j) { return tile_info(j).valid; };
             // Walk from tile nj to the slot's next used tile: an unused tile is released once its fills
             // have been observed; at a used tile, its K fill is awaited.  Non-blocking mode gives up at the
@@ -913,58 +918,90 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 ++n;
             }
         }
-        // ---- epilogue: O / l -> swizzled staging image in shared memory -> bulk copies to the slot's
-        // partial state (row r of the image: 32 chunks of 16 B, chunk c stored at position c ^ (r & 7)) ----
+        // ---- epilogue: O / l -> swizzled staging image in shared memory -> bulk copies to the partial
+        // state (row r of the image: 32 chunks of 16 B, chunk c stored at position c ^ (r & 7)).  A pair
+        // item writes one state per slot.  A split item first merges its two slots (two running states of
+        // the same rows over disjoint keys) in registers and writes ONE state: the exchange through L2
+        // carries 128 rows per CTA, not 256. ----
         mbar_wait(bar(kBarAllDone), 0);  // every MMA done: the ring is free for staging
         if (warp == 0 && lane == 0) TL(100);
+        const bool split = wk.mode == kModeSplit;
+        xm[(0 * 2 + h) * kTileM + rl] = l_run0;  // row sums of this half, both slots
+        xm[(1 * 2 + h) * kTileM + rl] = l_run1;
+        named_bar_sync(1, 256);
+        const float l_tot0 = l_run0 + xm[(0 * 2 + (h ^ 1)) * kTileM + rl];
+        const float l_tot1 = l_run1 + xm[(1 * 2 + (h ^ 1)) * kTileM + rl];
+        const int n_out = wk.mode == kModePair ? 2 : 1;
 #pragma unroll 1
-        for (int s = 0; s < 2; ++s) {
-            if (wk.mode == kModeSolo && s == 1) continue;
-            const float m_fin = s ? m_run1 : m_run0, l_fin = s ? l_run1 : l_run0;
-            const int rows_s = wk.rows(s);
-            const size_t prow0 = (size_t)wk.group * pl.grp_rows + wk.part_row0(s);
+        for (int o = 0; o < n_out; ++o) {
+            // out state o = w0 * O_slot0 + w1 * O_slot1 (use0 / use1 are uniform over the CTA: a slot
+            // without any unit holds an uninitialised accumulator and is not read at all)
+            bool use0, use1;
+            float w0, w1, lse_v;
+            int rows_o;
+            if (split) {
+                use0 = kcnt0 > 0;
+                use1 = kcnt1 > 0;
+                const float m0 = use0 ? m_run0 : -INFINITY, m1 = use1 ? m_run1 : -INFINITY;
+                const float m = fmaxf(m0, m1);
+                const float a0 = m0 == -INFINITY ? 0.f : ex2((m0 - m) * c2);
+                const float a1 = m1 == -INFINITY ? 0.f : ex2((m1 - m) * c2);
+                const float l = a0 * l_tot0 + a1 * l_tot1;
+                const float inv = l > 0.f ? 1.f / l : 0.f;  // l = 0: every key of the chunk masked
+                w0 = a0 * inv;
+                w1 = a1 * inv;
+                lse_v = l > 0.f ? m * pl.sm_scale + logf(l) : -INFINITY;
+                rows_o = wk.rows0;
+            } else {
+                const bool any = (o ? kcnt1 : kcnt0) > 0;  // false: empty chunk 0 -> state (0, -inf)
+                use0 = any && o == 0;
+                use1 = any && o == 1;
+                const float lt = o ? l_tot1 : l_tot0, mf = o ? m_run1 : m_run0;
+                const float inv = any && lt > 0.f ? 1.f / lt : 0.f;
+                w0 = use0 ? inv : 0.f;
+                w1 = use1 ? inv : 0.f;
+                lse_v = any && lt > 0.f ? mf * pl.sm_scale + logf(lt) : -INFINITY;
+                rows_o = wk.rows(o);
+            }
+            const size_t prow0 = (size_t)wk.group * pl.grp_rows + wk.part_row0(o);
             float* po = a.part_o + prow0 * kD;
             float* plse = a.part_lse + prow0;
-            const bool row_ok = rl < rows_s;
-            if ((s ? kcnt1 : kcnt0) == 0) {  // no unit for this slot (empty chunk 0, or a split chunk of a single key tile)
-                if (h == 0 && row_ok) plse[rl] = -INFINITY;
-                if (row_ok)  // the merge reads every state's O unguarded: give it zeros (weight 0 anyway)
-                    for (int c = h * 16; c < h * 16 + 16; ++c)
-                        reinterpret_cast<float4*>(po + (size_t)rl * kD)[c] = make_float4(0.f, 0.f, 0.f, 0.f);
-                continue;
-            }
-            const bool warp_active = w * 32 < rows_s;
-            xm[h * kTileM + rl] = l_fin;
-            named_bar_sync(1, 256);
-            const float l_tot = l_fin + xm[(h ^ 1) * kTileM + rl];
-            const uint32_t stage = smem + kOffRing + (uint32_t)s * (2 * kKvTileBytes);
+            const bool row_ok = rl < rows_o;
+            const bool warp_active = w * 32 < rows_o;
+            const uint32_t stage = smem + kOffRing + (uint32_t)o * (2 * kKvTileBytes);
             if (warp_active) {
                 tc_fence_after();
-                const float inv = l_tot > 0.f ? 1.f / l_tot : 0.f;  // l = 0: every key of the chunk masked
                 const uint32_t srow = stage + (uint32_t)rl * 512u;
-                const uint32_t o_addr = tmem + s * kD + h * 64 + lane_addr;
+                const uint32_t o_addr = tmem + h * 64 + lane_addr;
 #pragma unroll
                 for (int c0 = 0; c0 < 64; c0 += 32) {
-                    uint32_t o[32];
-                    D2SD_TMEM_LD32(o_addr + c0, o, 0);
+                    uint32_t ov0[32], ov1[32];
+                    if (use0) D2SD_TMEM_LD32(o_addr + c0, ov0, 0);
+                    if (use1) D2SD_TMEM_LD32(o_addr + kD + c0, ov1, 0);
                     tmem_wait_ld();
+                    float acc[32];
+#pragma unroll
+                    for (int c = 0; c < 32; ++c) {
+                        acc[c] = use0 ? __uint_as_float(ov0[c]) * w0 : 0.f;
+                        if (use1) acc[c] += __uint_as_float(ov1[c]) * w1;
+                    }
 #pragma unroll
                     for (int c = 0; c < 32; c += 4) {
                         const uint32_t chunk = (uint32_t)((h * 64 + c0 + c) >> 2);
                         const uint32_t phys = chunk ^ ((uint32_t)rl & 7u);
-                        asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(srow + phys * 16u),
-                                     "f"(__uint_as_float(o[c]) * inv), "f"(__uint_as_float(o[c + 1]) * inv),
-                                     "f"(__uint_as_float(o[c + 2]) * inv), "f"(__uint_as_float(o[c + 3]) * inv)
+                        asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(srow + phys * 16u), "f"(acc[c]),
+                                     "f"(acc[c + 1]), "f"(acc[c + 2]), "f"(acc[c + 3])
                                      : "memory");
                     }
                 }
-                if (h == 0 && row_ok) plse[rl] = l_tot > 0.f ? m_fin * pl.sm_scale + logf(l_tot) : -INFINITY;
+                if (h == 0 && row_ok) plse[rl] = lse_v;
                 fence_async_smem();
             }
             named_bar_sync(1, 256);  // both halves of every row are staged
-            if (warp_active && h == (s & 1) && lane == 0) {
+            if (warp == 0 && lane == 0) TL(102 + o);
+            if (warp_active && h == (o & 1) && lane == 0) {
                 // this warp's rows: one contiguous piece of the image and of the partial state
-                const int nrows = min(32, rows_s - w * 32);
+                const int nrows = min(32, rows_o - w * 32);
                 bulk_store(po + (size_t)(w * 32) * kD, stage + (uint32_t)(w * 32) * 512u, (uint32_t)nrows * 512u);
                 bulk_commit();
             }

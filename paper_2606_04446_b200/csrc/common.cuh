@@ -69,7 +69,7 @@ int32_t launch_accept(const __nv_bfloat16* logits, int64_t row_stride, int V, co
 //  tcgen05 path (attn_cascade_sm100.cu): a header of self-resetting group counters (zero between
 //    calls), then partials per group (request, kv head, item): O fp32 [group][grp_rows][d] and LSE
 //    fp32 [group][grp_rows]; a pair item holds chunk c's two query tiles at rows c*256.., a single
-//    item holds (chunk c, key-tile parity s) at rows (2c+s)*128..; the tree keys are key tiles of
+//    item holds chunk c (its two key-parity states already merged) at rows c*128..; the tree keys are key tiles of
 //    the same kernel.
 struct AttnPlan {
     int B, T_cap, W, Hq, Hkv, G, d;
