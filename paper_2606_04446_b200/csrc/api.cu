@@ -1,7 +1,6 @@
 // extern "C" entry points of libd2sd (declared and documented in include/d2sd.h): argument checks,
 // launch planning, kernel enqueue.  No allocation, no synchronisation, no host reads of device data.
 #include <cmath>
-#include <cstdlib>
 #include <cstring>
 
 #include "common.cuh"
@@ -102,6 +101,8 @@ static int32_t make_plan(const d2sd_attn_params* p, AttnPlan* out) {
                 cb = budget / pl.n_single;
             }
         } else {
+            // more SMs' worth of (request, kv head) pairs than SMs: fixed chunks of ~32 key tiles (measured
+            // on config 5: 8 -> 467 us, 16 -> 379, 32 -> 363, 44 -> 359, 66 -> 413)
             ca = ceil_div(max_tiles, 32);
             cb = ceil_div(max_tiles, 64);
             pl.tps_min = -1;  // fixed below
