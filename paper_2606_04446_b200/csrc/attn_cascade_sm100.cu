@@ -148,7 +148,8 @@ __device__ __forceinline__ void named_bar_arrive(uint32_t id, uint32_t threads) 
 __device__ __forceinline__ void named_bar_sync(uint32_t id, uint32_t threads) {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
 }
-constexpr uint64_t kEvictFirst = 0x12F0000000000000ull;  // streamed: KV
+constexpr uint64_t kEvictNormal = 0x1000000000000000ull;  // KV: read by the 2-3 sibling CTAs of the kv head within a few
+                                                          // microseconds (evict-first measured 3% slower on configs 3, 4)
 constexpr uint64_t kEvictLast = 0x14F0000000000000ull;   // re-read by every chunk CTA of the head: Q
 
 // D[tmem] (+)= A[smem] . B[smem]
@@ -601,12 +602,12 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                     __syncwarp();
                     if (lane < 2 * n_pages)
                         tma_load_5d(dst + (uint32_t)(lane & 1) * (kKvTileBytes / 2) + (uint32_t)(lane >> 1) * 2048u,
-                                    kv ? &tm_v : &tm_k, bar(kBarFull + i), 0, 0, lane & 1, wk.g, page_cur, kEvictFirst);
+                                    kv ? &tm_v : &tm_k, bar(kBarFull + i), 0, 0, lane & 1, wk.g, page_cur, kEvictNormal);
                 } else if (lane == 0) {
                     mbar_wait(bar(kBarEmpty + i), ((x / kRing) & 1) ^ 1);
                     mbar_expect_tx(bar(kBarFull + i), kKvTileBytes);
                     const CUtensorMap* tm = ti.tree ? (kv ? &tm_tv : &tm_tk) : (kv ? &tm_v : &tm_k);
-                    tma_load_4d(dst, tm, bar(kBarFull + i), 0, ti.row, 0, wk.g, ti.tree ? kEvictLast : kEvictFirst);
+                    tma_load_4d(dst, tm, bar(kBarFull + i), 0, ti.row, 0, wk.g, ti.tree ? kEvictLast : kEvictNormal);
                 }
                 if (x == 0 && lane == 0) {
                     // a split item holds one M tile (Q buffer 0 serves both slots)
