@@ -7,14 +7,17 @@
 // (np = ceil(L/128)) and tree tiles np..np+nt-1 (nt = ceil(T/128)); the tree tiles are ordinary key
 // tiles whose scores additionally pass the node's ancestor-mask bits.
 //
-// Work decomposition.  M tiles (2p, 2p+1) form "pair item" p; an odd last M tile is the "single
-// item".  The key-tile sequence of the request is cut into chunks; one CTA serves (request b, kv
+// Work decomposition.  A query tile is either half of a "pair item" (tiles 2p, 2p+1) or a "split item"
+// of its own; the launch plan decides (api.cu: up to three query tiles in the one-wave regime are all
+// split items).  The key-tile sequence of the request is cut into chunks; one CTA serves (request b, kv
 // head g, item, chunk) and owns two accumulator SLOTS that strictly alternate in the unit stream
 // (one unit = one M tile x one 128-key tile):
 //
-//   pair item   : slot s = M tile 2p+s; every key tile of the chunk feeds both slots
-//   single item : both slots hold the same M tile; slot s takes the chunk's key tiles of parity s
-//                 (two running softmax states over disjoint keys, merged like any two chunks)
+//   pair item   : slot s = M tile 2p+s; every key tile of the chunk feeds both slots (the KV tile crosses
+//                 the L2->SM crossbar once per 256 query rows; two partial states leave the CTA)
+//   split item  : both slots hold the same M tile; slot s takes the chunk's key tiles of parity s
+//                 (two running softmax states over disjoint keys, merged in registers in the epilogue:
+//                 one partial state of 128 rows leaves the CTA)
 //
 // so that the tensor phase of one slot (P.V, then the next Q.K^T, which cannot start earlier because P
 // overwrites S in TMEM) runs under the other slot's softmax.  The eight softmax warps serve one unit
@@ -34,8 +37,8 @@
 // raised when a tile maximum exceeds it by more than 2^8 (lazy rescale), in which case the owning
 // thread rescales its O row in TMEM before the next P.V.
 //
-// Cascade merge in the same launch (log-sum-exp state merge): every CTA writes one
-// partial state (normalised O fp32, LSE) per slot to the workspace (bulk copies from a shared-memory
+// Cascade merge in the same launch (log-sum-exp state merge): every CTA writes its
+// partial state(s) (normalised O fp32, LSE) to the workspace (bulk copies from a shared-memory
 // staging image; it stays in L2), publishes it with a release-increment of its group's arrival
 // counter (group = request, kv head, item), waits until all non-empty chunks of the group have
 // arrived, and then merges ITS share of the group's rows and writes the bf16 output and the LSE.
