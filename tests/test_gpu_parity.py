@@ -165,8 +165,10 @@ def _ramp_keys(kv, ctx_len, lo=0.25, hi=4.0):
     kv["k_cache"] = synth.f32_to_bf16_bits(k)
 
 
-def _attn_full_case(d2sd, oracle, cfg, q_scale=1.0, layer=0, pool_nan=False, ramp=False, **kw):
+def _attn_full_case(d2sd, oracle, cfg, q_scale=1.0, layer=0, pool_nan=False, ramp=False, conf=None, **kw):
     st = synth.make_step_inputs(cfg)
+    if conf is not None:
+        st["conf"][:] = np.asarray(conf, dtype=np.float32)
     _, _, tree = oracle_tree(oracle, cfg, st)
     ti = synth.make_tree_inputs(cfg, layer, q_scale=q_scale)
     kv = synth.make_kv_cache(cfg, st["ctx_len"], layer, pool_fill_nan=pool_nan)
@@ -250,6 +252,21 @@ def test_attn_paged_ragged_reduced_config5(d2sd, oracle, impl, ctx):
     contexts; slots no request owns are NaN and must never reach an output."""
     cfg = synth.custom(91, B=6, gamma=16, K=4, ctx=ctx, paged=True)
     _attn_full_case(d2sd, oracle, cfg, pool_nan=True, impl=impl)
+
+
+@pytest.mark.parametrize("L", [300, 2500])
+def test_attn_short_tree_in_pair_plan(d2sd, oracle, L):
+    """Config-4 shape (T_cap = 252: eight query tiles, planned as four pair items) with confidences that
+    select the eight longest prefixes, so the tree has 76 nodes = 304 query rows: pair item 0 is full,
+    pair item 1 holds 48 rows in its first tile and none in its second (it runs as a split item in the
+    pair item's partial-state layout), pair items 2 and 3 are idle."""
+    cfg = synth.custom(92, gamma=32, K=8, ctx=(L, L))
+    conf = np.full(cfg.gamma, 0.5, dtype=np.float32)
+    conf[:23] = 1.0
+    o, lse = _attn_full_case(d2sd, oracle, cfg, conf=conf)
+    st = synth.make_step_inputs(cfg)
+    st["conf"][:] = conf
+    assert int(oracle_tree(oracle, cfg, st)[2]["tree_len"][0]) == 76
 
 
 @pytest.mark.parametrize("impl", IMPLS)
