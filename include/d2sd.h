@@ -102,9 +102,9 @@ int32_t d2sd_build_tree(const int32_t* draft1, const int32_t* draft2, const int3
  * computed as a cascade: all T*G query rows of one kv head share one pass over that head's prefix
  * KV (streamed from HBM once), split along the context into `num_splits` chunks with a partial
  * (O, LSE) per chunk; the <= T_cap tree keys are attended under the ancestor mask; all partial
- * states are merged by log-sum-exp.  Contiguous KV with 128 % G == 0 runs as ONE fused tcgen05
- * launch (tree keys = extra key tiles, merge in the same kernel); other shapes run the mma.sync
- * kernels (prefix/tree pass + merge).  bf16 in, fp32 accumulate, bf16 out.  Q and tree K are taken post q/k-norm and
+ * states are merged by log-sum-exp.  Contiguous or 16-key-paged KV with 128 % G == 0 runs as ONE fused
+ * tcgen05 launch (tree keys = extra key tiles, merge in the same kernel); other group sizes run the
+ * mma.sync kernels (prefix/tree pass + merge).  bf16 in, fp32 accumulate, bf16 out.  Q and tree K are taken post q/k-norm and
  * post-RoPE (pos_id from (b) is for the caller's RoPE).  No sliding window / sinks / soft-cap.
  * ------------------------------------------------------------------------------------------- */
 typedef struct d2sd_attn_params {
