@@ -122,7 +122,7 @@ accept_walk_kernel(const ArgPart* __restrict__ part, int n_chunks, const int32_t
             int bi = INT_MAX;
             const ArgPart* p = part + o * n_chunks;
             for (int c = 0; c < n_chunks; ++c) arg_update(p[c].v, p[c].i, bv, bi);
-            a = bi;
+            a = bi == INT_MAX ? 0 : bi;  // a row of NaNs only: index 0, never an out-of-range token id
             par_s[n] = parent[o];
             tok_s[n] = tokens[o];
         }

@@ -19,12 +19,15 @@ int32_t set_error(int32_t status, const char* fmt, ...) {
 void clear_error() { g_err[0] = '\0'; }
 
 int sm_count() {
-    static int n = 0;
+    // per device (a process may drive several GPUs); a benign race at worst writes the same value twice
+    static int cache[64] = {0};
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return 148;  // B200
+    if (dev < 0 || dev >= 64) dev = 0;
+    int n = cache[dev];
     if (n == 0) {
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess ||
-            cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0)
-            n = 148;  // B200
+        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
+        cache[dev] = n;
     }
     return n;
 }
@@ -122,8 +125,12 @@ static int32_t make_plan(const d2sd_attn_params* p, AttnPlan* out) {
         pl.grp_rows = 256 * (pl.n_pair ? (pl.n_single && cb > ca ? cb : ca) : cb);
         const size_t n_groups = (size_t)pl.B * pl.Hkv * (pl.n_pair + pl.n_single);
         const size_t slot_rows = n_groups * pl.grp_rows;
+        // The counter header has a FIXED size, so that one workspace can serve calls with different
+        // params one after another (the scratch of one call never lands on the counters of another).
+        D2SD_CHECK_SUPPORTED(n_groups * 2 * sizeof(unsigned) <= kWsHeaderBytes, "B*Hkv*items = %zu groups > %zu",
+                             n_groups, kWsHeaderBytes / (2 * sizeof(unsigned)));
         pl.off_cnt = 0;
-        pl.cnt_bytes = align_up(n_groups * 2 * sizeof(unsigned), 256);
+        pl.cnt_bytes = kWsHeaderBytes;
         pl.off_o = pl.cnt_bytes;
         pl.off_lse = pl.off_o + align_up(slot_rows * pl.d * sizeof(float), 256);
         pl.bytes = pl.off_lse + align_up(slot_rows * sizeof(float), 256);
@@ -143,9 +150,9 @@ static int32_t make_plan(const d2sd_attn_params* p, AttnPlan* out) {
         pl.NS = pl.num_splits + 1;
         const size_t rows_all = (size_t)pl.B * pl.NS * pl.T_cap * pl.Hq;
         pl.off_cnt = 0;
-        pl.cnt_bytes = 0;
-        pl.off_o = 0;
-        pl.off_lse = align_up(rows_all * pl.d * sizeof(float), 256);
+        pl.cnt_bytes = kWsHeaderBytes;  // unused by these kernels, but never overwritten either
+        pl.off_o = pl.cnt_bytes;
+        pl.off_lse = pl.off_o + align_up(rows_all * pl.d * sizeof(float), 256);
         pl.bytes = pl.off_lse + align_up(rows_all * sizeof(float), 256);
     }
     *out = pl;
@@ -205,6 +212,9 @@ int32_t d2sd_cascade_verify_attn(const d2sd_attn_params* p, const void* q, const
     if (pl.B == 0) return D2SD_OK;
     D2SD_CHECK_ARG(q && ctx_len && tree_k && tree_v && mask && tree_len && out, "a required buffer is NULL");
     D2SD_CHECK_ARG(p->max_ctx_len == 0 || (k_cache && v_cache), "k_cache / v_cache is NULL");
+    D2SD_CHECK_ARG(p->max_ctx_len == 0 || p->kv_rows > 0, "max_ctx_len = %d but kv_rows = 0", p->max_ctx_len);
+    D2SD_CHECK_ARG(p->page_size == 0 || p->kv_rows % p->page_size == 0, "kv_rows = %lld is not a whole number of pages",
+                   (long long)p->kv_rows);
     D2SD_CHECK_ARG(kv_indptr != nullptr || (pl.B == 1 && pl.page_size == 0),
                    "kv_indptr may be NULL only for B == 1 contiguous KV");
     D2SD_CHECK_ARG((pl.page_size > 0) == (kv_indices != nullptr),

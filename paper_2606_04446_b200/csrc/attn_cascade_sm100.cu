@@ -297,23 +297,6 @@ __device__ __forceinline__ void bulk_store(void* gdst, uint32_t ssrc, uint32_t b
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 
-#ifdef D2SD_TIMELINE
-// Debug builds only (-DD2SD_TIMELINE): per-CTA cycle stamps of pipeline events, read back with
-// d2sd_debug_timeline().  Not part of the C ABI.
-__device__ long long g_timeline[256][128];
-#define TL(slot)                                                                                    \
-    do {                                                                                            \
-        const int _c = blockIdx.x + gridDim.x * blockIdx.y;                                         \
-        if (_c < 256 && (slot) < 128) g_timeline[_c][(slot)] = clock64() - tl_t0;                   \
-    } while (0)
-// accumulate the cycles since the previous TLA of this thread into bucket `b` (dumped at slots 3..15)
-#define TLA(b) do { const long long _t = clock64(); tl_acc[(b)] += _t - tl_last; tl_last = _t; } while (0)
-#define TLABS(slot) do { if (warp == 0 && lane == 0) { const int _c = blockIdx.x + gridDim.x * blockIdx.y; if (_c < 256) g_timeline[_c][(slot)] = clock64(); } } while (0)
-#else
-#define TLABS(slot) do {} while (0)
-#define TL(slot) do {} while (0)
-#define TLA(b) do {} while (0)
-#endif
 
 // What one CTA does: which item / chunk, which rows its two slots hold, which key tiles it streams.
 enum : int { kModePair = 0, kModeSplit = 2 };
@@ -390,7 +373,6 @@ __device__ __forceinline__ void merge_rows(const AttnPlan& pl, const AttnArgs& a
         lse_sm[e] = v;
     }
     named_bar_sync(1, 256);
-    TLABS(110);
     auto out_row = [&](int r) {  // index of query row r0 + r of the item in out / lse: [b][t][h]
         const int ra = wk.row_base + r0 + r, t = ra / G;
         return ((size_t)wk.b * pl.T_cap + t) * pl.Hq + wk.g * G + (ra - t * G);
@@ -420,7 +402,6 @@ __device__ __forceinline__ void merge_rows(const AttnPlan& pl, const AttnArgs& a
     }
     named_bar_sync(1, 256);
     mbar_wait(bar_merge, 0);  // the O rows have landed
-    TLABS(111);
     // step 2, one thread per (row, 16-byte chunk): O = sum_p weight_p O_p.  States without any key hold
     // zeros (their CTA wrote them), so no value needs guarding.
 #pragma unroll 1
@@ -449,7 +430,6 @@ __device__ __forceinline__ void merge_rows(const AttnPlan& pl, const AttnArgs& a
         pk.y = *reinterpret_cast<uint32_t*>(&hi);
         *reinterpret_cast<uint2*>(a.out + orow * kD + col) = pk;
     }
-    TLABS(113);
 }
 
 // mode bits: 1 = include the prefix tiles, 2 = include the tree tiles (3 = the whole cascade).
@@ -499,9 +479,6 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
     }
     pdl_launch_dependents();  // the next kernel may begin its own prologue as SMs free up
     pdl_wait();               // everything before this kernel in the stream is complete and visible
-#ifdef D2SD_TIMELINE
-    const long long tl_t0 = clock64();
-#endif
 
     // ---- this CTA's work ----
     Work wk;
@@ -562,10 +539,6 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
-    if (tid == 0) TL(0);
-#ifdef D2SD_TIMELINE
-    if (tid == 0) g_timeline[blockIdx.x + gridDim.x * blockIdx.y][123] = tl_t0;
-#endif
 
     // the control warpgroup hands registers to the two softmax warpgroups (one instruction per warpgroup)
     if (warp >= 8) {
@@ -640,10 +613,6 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             const uint32_t sd = tmem + kTmemS + s * kTileN;  // S, overwritten by P (bf16, 64 columns)
             const uint32_t od = tmem + s * kD;
             uint32_t acc = 0, par = 0, n_ragged = 0;
-#ifdef D2SD_TIMELINE
-            long long tl_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0}, tl_last = clock64();
-            int n = 0;
-#endif
             int jj = 0, ki = 0, kpar = 0;  // current tile and the ring slot / fill parity of its K
             auto ring_next = [&](int& i, int& p) { if (++i == kRing) { i = 0; p ^= 1; } };
             auto is_used = [&](int j) { return ((wk.uses(j) >> s) & 1u) != 0; };
@@ -689,12 +658,7 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             jj = nj; ki = nki; kpar = nkpar;
             if (jj < wk.n_tiles) {
                 mbar_wait(bar(kBarQFull + (wk.mode == kModePair ? s : 0)), 0);
-                TLA(5);
-#ifdef D2SD_TIMELINE
-                TL(16 + 3 * s);
-#endif
                 issue_qk(jj, ki);
-                TLA(6);
             }
             while (jj < wk.n_tiles) {
                 const int valid = valid_of(jj);
@@ -703,18 +667,15 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 ring_next(vi, vpar);
                 mbar_wait(bar(kBarFull + vi), vpar);
                 if (valid & 15) mbar_wait(bar(kBarVFix + n_ragged++), 0);
-                TLA(1);  // V wait
                 // the next unit of this slot and its K tile, before the P pieces arrive
                 nj = jj + 1; nki = vi; nkpar = vpar; nsub = 0;
                 ring_next(nki, nkpar);
                 const bool next_ready = advance(false);
-                TLA(5);  // K wait
                 const uint64_t vd = smem_desc(smem + kOffRing + vi * kKvTileBytes, kKvTileBytes / 2, 1024);
 #pragma unroll
                 for (int q = 0; q < 4; ++q) {
                     if (2 * q < ksteps) {
                         mbar_wait(bar(kBarPFull + 4 * s + q), par);
-                        TLA(2);  // P wait
                         tc_fence_after();
 #pragma unroll
                         for (int ks = 2 * q; ks < 2 * q + 2; ++ks)
@@ -723,30 +684,12 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 }
                 acc = 1;
                 par ^= 1;
-                TLA(3);  // P.V issue
-#ifdef D2SD_TIMELINE
-                if (n < 8) TL(16 + 6 * n + 3 * s + 2);
-                ++n;
-#endif
                 tc_commit(bar(kBarEmpty + vi));  // V_j is free once these P.V pieces have completed
-                TLA(4);
                 if (!next_ready) advance(true);
-                TLA(5);
-#ifdef D2SD_TIMELINE
-                if (nj < wk.n_tiles && n < 8) TL(16 + 6 * n + 3 * s);
-#endif
                 if (nj < wk.n_tiles) issue_qk(nj, nki);
-                TLA(6);  // Q.K^T issue
                 jj = nj; ki = nki; kpar = nkpar;
             }
             tc_commit(bar(kBarAllDone));
-#ifdef D2SD_TIMELINE
-            TLA(0);
-            for (int i = 0; i < 7; ++i) {
-                const int _c = blockIdx.x + gridDim.x * blockIdx.y;
-                if (_c < 256 && s == 0) g_timeline[_c][3 + i] = tl_acc[i];
-            }
-#endif
         }
       } else if (warp == 11) {
         // ===== V sanitiser: the P.V MMA runs over ceil16(valid) keys; rows valid..ceil16(valid)-1 of a
@@ -809,15 +752,10 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 if (!((use >> s) & 1u)) continue;
                 const int k = s ? kcnt1 : kcnt0;
                 float m_cur = s ? m_run1 : m_run0, l_cur = s ? l_run1 : l_run0;
-#ifdef D2SD_DBG_NOSOFTMAX
-                const bool warp_active = false;  // timing experiment only: results are garbage
-#else
                 const bool warp_active = w * 32 < wk.rows(s);
-#endif
                 const uint32_t sbuf = tmem + kTmemS + s * kTileN + lane_addr;
                 const uint32_t o_addr = tmem + s * kD + h * 64 + lane_addr;
                 mbar_wait(bar(kBarSFull + s), k & 1);
-                if (warp == 0 && lane == 0 && n < 16) TL(64 + 2 * n);
                 uint32_t sv[64];
                 float mxh = -INFINITY;
                 if (warp_active) {
@@ -917,7 +855,6 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                     mbar_arrive(bar(kBarPFull + 4 * s + 2 * h));
                     mbar_arrive(bar(kBarPFull + 4 * s + 2 * h + 1));
                 }
-                if (warp == 0 && lane == 0 && n < 16) TL(64 + 2 * n + 1);
                 if (s) { m_run1 = m_cur; l_run1 = l_cur; ++kcnt1; } else { m_run0 = m_cur; l_run0 = l_cur; ++kcnt0; }
                 ++n;
             }
@@ -928,7 +865,6 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
         // the same rows over disjoint keys) in registers and writes ONE state: the exchange through L2
         // carries 128 rows per CTA, not 256. ----
         mbar_wait(bar(kBarAllDone), 0);  // every MMA done: the ring is free for staging
-        if (warp == 0 && lane == 0) TL(100);
         const bool split = wk.mode == kModeSplit;
         xm[(0 * 2 + h) * kTileM + rl] = l_run0;  // row sums of this half, both slots
         xm[(1 * 2 + h) * kTileM + rl] = l_run1;
@@ -1002,7 +938,6 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 fence_async_smem();
             }
             named_bar_sync(1, 256);  // both halves of every row are staged
-            if (warp == 0 && lane == 0) TL(102 + o);
             if (warp_active && h == (o & 1) && lane == 0) {
                 // this warp's rows: one contiguous piece of the image and of the partial state
                 const int nrows = min(32, rows_o - w * 32);
@@ -1015,7 +950,6 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             asm volatile("fence.proxy.async;" ::: "memory");
         }
         __syncwarp();
-        if (warp == 0 && lane == 0) TL(101);
 
         // ---- publish this CTA's partial states, wait for the group, merge this CTA's share of rows ----
         const unsigned expected = (unsigned)wk.n_chunks;
@@ -1036,7 +970,6 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             done_before = atomicAdd(cnt + 1, 1u);
         }
         named_bar_sync(1, 256);
-        if (warp == 0 && lane == 0) TL(120);
         asm volatile("fence.proxy.async;" ::: "memory");  // the bulk copies below read what the acquire made visible
         merge_rows(pl, a, dbg_rows, wk, smem + kOffQ, smem_gen + kOffQ, bar(kBarMerge), warp, lane);
         if (warp == 0 && lane == 0) {
@@ -1044,14 +977,12 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 cnt[0] = 0;
                 cnt[1] = 0;
             }
-            TL(121);
         }
       }
     }
 
     tc_fence_before();
     __syncthreads();
-    if (tid == 0) TL(2);
     if (warp == 10) {
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(kTmemCols) : "memory");
     }
@@ -1096,12 +1027,10 @@ bool attn_cascade_tc_supported(const AttnPlan& pl) {
 }
 
 int32_t launch_attn_cascade_tc(const AttnPlan& pl, const AttnArgs& a, int mode, float* dbg_rows, cudaStream_t s) {
-    static bool attr_set = false;
-    if (!attr_set) {
+    static unsigned long long attr_done = 0;
+    if (first_use_on_device(attr_done))
         D2SD_CHECK_CUDA(cudaFuncSetAttribute(attn_cascade_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              (int)kSmemBytes));
-        attr_set = true;
-    }
     CUtensorMap tm_q, tm_k, tm_v, tm_tk, tm_tv;
     {   // Q [B*T_cap, Hq, d] viewed as (d_lo 64, hh G, t B*T_cap, d_hi 2, g Hkv): one box = one 128-row query tile
         const cuuint64_t dims[5] = {64, (cuuint64_t)pl.G, (cuuint64_t)pl.B * pl.T_cap, 2, (cuuint64_t)pl.Hkv};
@@ -1150,10 +1079,5 @@ int32_t launch_attn_cascade_tc(const AttnPlan& pl, const AttnArgs& a, int mode, 
     return D2SD_OK;
 }
 
-#ifdef D2SD_TIMELINE
-extern "C" int32_t d2sd_debug_timeline(long long* host_buf /* [256][128] */) {
-    return cudaMemcpyFromSymbol(host_buf, g_timeline, sizeof(long long) * 256 * 128) == cudaSuccess ? 0 : -4;
-}
-#endif
 
 }  // namespace d2sd

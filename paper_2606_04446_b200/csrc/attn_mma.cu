@@ -1,7 +1,8 @@
 // Stage (c), generic path: split-KV flash attention on mma.sync (m16n8k16 bf16, fp32 accumulate).
-// Serves (1) the tree pass of every configuration -- <= T_cap keys under the ancestor mask, far too
-// small for tcgen05 tiles -- and (2) the prefix pass for shapes the tcgen05 kernel does not cover
-// (paged KV, G not dividing 128) or when impl=1 forces it.  PAPER.md:52, :124, :154.
+// Serves the shapes the fused tcgen05 kernel (attn_cascade_sm100.cu) does not cover -- GQA group sizes
+// that do not divide a 128-row query tile -- and impl = 1 (tests: an independent second CUDA path):
+// prefix chunks and the tree pass (<= T_cap keys under the ancestor mask) as one launch, merge as a
+// second.  Contiguous and paged KV.  PAPER.md:52, :124, :154.
 //
 // CTA = 4 warps x 16 query rows = 64 rows of one (request, kv head); rows are the flattened
 // (tree node t, head-in-group) pairs r = t*G + hh so that all GQA heads and all branches share one
@@ -351,12 +352,10 @@ __global__ void __launch_bounds__(128) attn_merge_kernel(AttnPlan pl, AttnArgs a
 
 int32_t launch_attn_mma(const AttnPlan& pl, const AttnArgs& a, bool do_prefix, bool do_tree,
                         cudaStream_t s) {
-    static bool attr_set = false;
-    if (!attr_set) {
+    static unsigned long long attr_done = 0;
+    if (first_use_on_device(attr_done))
         D2SD_CHECK_CUDA(cudaFuncSetAttribute(attn_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              SMEM_BYTES));
-        attr_set = true;
-    }
     const int first = do_prefix ? 0 : pl.num_splits;
     const int last = do_tree ? pl.num_splits : pl.num_splits - 1;
     if (last < first) return D2SD_OK;

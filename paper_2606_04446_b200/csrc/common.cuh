@@ -47,7 +47,17 @@ void clear_error();
 inline int ceil_div(int a, int b) { return (a + b - 1) / b; }
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
-int sm_count();  // cached multiprocessor count of the current device
+int sm_count();  // multiprocessor count of the current device (cached per device)
+// True exactly once per device and call site (per-device function attributes such as the dynamic shared
+// memory opt-in); a race between two first callers only repeats an idempotent call.
+inline bool first_use_on_device(unsigned long long& done_mask) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return true;
+    if ((done_mask >> dev) & 1ull) return false;
+    done_mask |= 1ull << dev;
+    return true;
+}
+constexpr size_t kWsHeaderBytes = 1u << 20;  // fixed-size head of the attention workspace (group counters)
 
 // ---- stage launchers (defined in the per-stage .cu files) -------------------------------------
 int32_t launch_select(const float* conf, int B, int gamma, int K, int32_t* prefix_len, double* r_out,

@@ -95,12 +95,12 @@ def _accept_case(d2sd, oracle, cfg, logits_bits, tree, gamma, row_stride=None):
     return ref
 
 
-@pytest.mark.parametrize("cfg_no", [1, 2, 4])
+@pytest.mark.parametrize("cfg_no", [1, 2, 3, 4, 5])
 def test_accept_bit_exact_configs(d2sd, oracle, cfg_no):
     cfg = synth.CONFIGS[cfg_no]
     st = synth.make_step_inputs(cfg)
     _, _, tree = oracle_tree(oracle, cfg, st)
-    for force in (None, 0.0, 1.0):
+    for force in ((None, 0.0, 1.0) if cfg.B * cfg.T_cap * cfg.V < (1 << 27) else (None,)):
         logits = synth.make_logits(cfg)
         synth.plant_acceptance(cfg, logits, st["conf"], tree["tokens"], tree["parent"], tree["depth"],
                                tree["tree_len"], force=force)
@@ -276,62 +276,183 @@ def test_attn_config2_one_layer_full(d2sd, oracle, impl):
     _attn_full_case(d2sd, oracle, cfg, layer=3, impl=impl)
 
 
-def _attn_sampled_case(d2sd, oracle, cfg, n_samples, layer=0):
+def test_attn_config3_full(d2sd, oracle):
+    """Config 3 (L = 32768, one of its 36 layers): every output element, plus both partial states."""
+    _attn_full_case(d2sd, oracle, synth.CONFIGS[3], layer=1)
+
+
+def test_attn_config4_full(d2sd, oracle):
+    """Config 4 (T_cap = 252, L = 8192: four pair items, several chunks each): every output element."""
+    _attn_full_case(d2sd, oracle, synth.CONFIGS[4])
+
+
+def test_attn_config5_full(d2sd, oracle):
+    """Config 5 (16 requests, paged, ragged 1024..16384): every output element of every request --
+    the only full-size case in the multi-wave regime of the launch plan."""
+    _attn_full_case(d2sd, oracle, synth.CONFIGS[5])
+
+
+@pytest.mark.parametrize("impl", IMPLS)
+def test_attn_multiwave_reduced(d2sd, oracle, impl):
+    """More (request, kv head) pairs than SMs (B*Hkv = 320 > 148) at a size the oracle finishes in
+    seconds: the multi-wave regime of the plan (fixed-length chunks), paged and ragged, every row."""
+    cfg = synth.custom(93, B=40, gamma=16, K=4, ctx=(100, 400), paged=True)
+    _attn_full_case(d2sd, oracle, cfg, pool_nan=True, impl=impl)
+
+
+def test_attn_multiwave_reduced_long(d2sd, oracle):
+    """Same regime with contexts long enough for several chunks per request (contiguous KV)."""
+    cfg = synth.custom(94, B=24, gamma=16, K=4, ctx=(3000, 9000))
+    _attn_full_case(d2sd, oracle, cfg)
+
+
+def _random_tree_mask(rng, B, T_cap, tree_len):
+    """Harness-side input: a random forest-free tree per request (parent[n] uniform in [0,n)), its
+    ancestor-closed mask by parent chasing.  Not the D2SD two-range shape: branches of branches."""
+    W = (T_cap + 31) // 32
+    mask = np.zeros((B, T_cap, W), np.uint32)
+    for b in range(B):
+        parent = np.full(T_cap, -1, np.int64)
+        for n in range(1, int(tree_len[b])):
+            parent[n] = rng.integers(0, n)
+        for n in range(int(tree_len[b])):
+            a = n
+            while a >= 0:
+                mask[b, n, a // 32] |= np.uint32(1 << (a % 32))
+                a = parent[a]
+    return mask
+
+
+@pytest.mark.parametrize("impl", IMPLS)
+@pytest.mark.parametrize("T_cap,L", [(70, 700), (252, 1300), (33, 0)])
+def test_attn_generic_ancestor_closed_mask(d2sd, oracle, impl, T_cap, L):
+    """include/d2sd.h: "any ancestor-closed mask whose row n has its self bit and no bit > n is
+    accepted" -- random trees (depth-3 and deeper, PAPER.md:228-240 is one such shape)."""
+    rng = np.random.default_rng(4000 + T_cap)
+    cfg = synth.custom(95, B=3, gamma=16, K=4, ctx=(L, L))
+    B = cfg.B
+    tree_len = np.array([T_cap, max(1, T_cap // 2), max(1, T_cap - 3)], np.int32)
+    mask = _random_tree_mask(rng, B, T_cap, tree_len)
     st = synth.make_step_inputs(cfg)
-    _, _, tree = oracle_tree(oracle, cfg, st)
-    ti = synth.make_tree_inputs(cfg, layer)
-    kv = synth.make_kv_cache(cfg, st["ctx_len"], layer)
-    o, lse, dbg = gpu_attention(d2sd, cfg, st, tree, ti, kv, dbg=True)
-    sel = synth.sample_rows(cfg, tree["tree_len"], n_samples)
+    big = synth.custom(95, B=B, gamma=64, K=16, ctx=(L, L))  # only its T_cap >= 252 sized tensors are used
+    ti = {k: v[:, :T_cap].copy() for k, v in synth.make_tree_inputs(big).items()}
+    kv = synth.make_kv_cache(cfg, st["ctx_len"])
+    tree = {"mask": mask, "tree_len": tree_len}
+    o, lse, dbg = gpu_attention(d2sd, cfg, st, tree, ti, kv, dbg=True, impl=impl)
     args = (ti["q"], kv["k_cache"], kv["v_cache"], kv["kv_indptr"], kv["kv_indices"], kv["page_size"],
-            st["ctx_len"], ti["tree_k"], ti["tree_v"], tree["mask"], sel)
-    ro, rl = oracle.attention_rows(*args, which="full")
-    b, t, h = sel[:, 0], sel[:, 1], sel[:, 2]
-    check_rows(o[b, t, h], lse[b, t, h], ro, rl, f"cfg{cfg.number} sampled full")
-    for idx, which in ((0, "prefix"), (1, "tree")):
-        so, sl = oracle.attention_rows(*args, which=which)
-        check_rows(dbg[idx][b, t, h][..., :-1], dbg[idx][b, t, h][..., -1], so, sl,
-                   f"cfg{cfg.number} sampled {which}-only", row_gate=STATE_REL_L2, elementwise=False)
-    v = valid_rows(tree["tree_len"], cfg.T_cap)
-    assert np.isfinite(o[v]).all() and np.isfinite(lse[v]).all()
-    assert np.isnan(o[~v]).all()
+            st["ctx_len"], ti["tree_k"], ti["tree_v"], mask, tree_len)
+    ro, rl = oracle.attention(*args, which="full")
+    v = valid_rows(tree_len, T_cap)
+    check_rows(o[v], lse[v], ro[v], rl[v], "generic mask full")
+    so, sl = oracle.attention(*args, which="tree")
+    check_rows(dbg[1][v][..., :-1], dbg[1][v][..., -1], so[v], sl[v], "generic mask tree-only",
+               row_gate=STATE_REL_L2, elementwise=False)
 
 
-def test_attn_config3_sampled(d2sd, oracle):
-    _attn_sampled_case(d2sd, oracle, synth.CONFIGS[3], 96)
+def test_attn_workspace_reuse_across_params(d2sd, oracle):
+    """include/d2sd.h: one initialised workspace serves calls with different params one after another
+    (varying B, T_cap, context, impl), as a serving loop with a max-size workspace does."""
+    cases = [synth.custom(96, B=4, gamma=16, K=4, ctx=(200, 900)),
+             synth.custom(97, B=1, gamma=16, K=4, ctx=(1500, 1500)),
+             synth.custom(98, B=2, gamma=32, K=8, ctx=(600, 700)),
+             synth.custom(96, B=4, gamma=16, K=4, ctx=(200, 900))]
+    impls = [0, 0, 1, 0, 0, 1, 0, 0]
+    need = max(d2sd.cascade_workspace_bytes(c.B, c.T_cap, c.Hq, c.Hkv, c.d, c.ctx[1], kv_rows=1 << 16, impl=i)
+               for c in cases for i in (0, 1))
+    ws = torch.empty(need + 4096, dtype=torch.uint8, device="cuda")
+    big = cases[0]
+    d2sd.cascade_workspace(big.B, big.T_cap, big.Hq, big.Hkv, big.d, big.ctx[1])  # smoke: allocate+init API
+    import ctypes
+    p = d2sd.binding._AttnParams(B=big.B, T_cap=big.T_cap, Hq=big.Hq, Hkv=big.Hkv, d=big.d, sm_scale=0.0, page_size=0,
+                                 max_ctx_len=big.ctx[1], kv_rows=1 << 16, num_splits=0, impl=0, phases=0)
+    assert d2sd.lib().d2sd_cascade_workspace_init(ctypes.byref(p), ws.data_ptr(), ws.numel(),
+                                                  torch.cuda.current_stream().cuda_stream) == 0
+    for rnd in range(2):
+        for cfg, impl in zip(cases, impls[rnd * 4:rnd * 4 + 4]):
+            st = synth.make_step_inputs(cfg)
+            _, _, tree = oracle_tree(oracle, cfg, st)
+            ti = synth.make_tree_inputs(cfg)
+            kv = synth.make_kv_cache(cfg, st["ctx_len"])
+            o, lse, _ = gpu_attention(d2sd, cfg, st, tree, ti, kv, impl=impl, workspace=ws)
+            ro, rl = oracle.attention(ti["q"], kv["k_cache"], kv["v_cache"], kv["kv_indptr"], None, 0, st["ctx_len"],
+                                      ti["tree_k"], ti["tree_v"], tree["mask"], tree["tree_len"])
+            v = valid_rows(tree["tree_len"], cfg.T_cap)
+            check_rows(o[v], lse[v], ro[v], rl[v], f"workspace reuse round {rnd} B={cfg.B} impl={impl}")
 
 
-def test_attn_config4_sampled(d2sd, oracle):
-    _attn_sampled_case(d2sd, oracle, synth.CONFIGS[4], 192)
-
-
-def test_attn_config5_sampled(d2sd, oracle):
-    _attn_sampled_case(d2sd, oracle, synth.CONFIGS[5], 128)
+def test_attn_two_streams_two_workspaces(d2sd, oracle):
+    """include/d2sd.h: two calls that may run concurrently need two workspaces -- and then work."""
+    cfgs = [synth.custom(99, B=2, gamma=16, K=4, ctx=(2500, 3000)), synth.custom(100, B=3, gamma=16, K=4, ctx=(1000, 2000))]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    jobs = []
+    for cfg in cfgs:
+        st = synth.make_step_inputs(cfg)
+        _, _, tree = oracle_tree(oracle, cfg, st)
+        ti = synth.make_tree_inputs(cfg)
+        kv = synth.make_kv_cache(cfg, st["ctx_len"])
+        dev = dict(q=bf16_cuda(ti["q"]), k=bf16_cuda(kv["k_cache"]), v=bf16_cuda(kv["v_cache"]),
+                   indptr=i32_cuda(kv["kv_indptr"]), ctx=i32_cuda(st["ctx_len"]), tk=bf16_cuda(ti["tree_k"]),
+                   tv=bf16_cuda(ti["tree_v"]), mask=mask_cuda(tree["mask"]), tl=i32_cuda(tree["tree_len"]),
+                   ws=d2sd.cascade_workspace(cfg.B, cfg.T_cap, cfg.Hq, cfg.Hkv, cfg.d, int(st["ctx_len"].max()),
+                                             kv_rows=int(kv["k_cache"].shape[0])))
+        jobs.append((cfg, st, tree, ti, kv, dev))
+    torch.cuda.synchronize()
+    results = [[], []]
+    for rep in range(6):  # interleave launches of the two streams
+        for i, (cfg, st, tree, ti, kv, dev) in enumerate(jobs):
+            with torch.cuda.stream(streams[i]):
+                results[i].append(d2sd.cascade_verify_attn(dev["q"], dev["k"], dev["v"], dev["indptr"], None, dev["ctx"],
+                                                           dev["tk"], dev["tv"], dev["mask"], dev["tl"],
+                                                           int(st["ctx_len"].max()), workspace=dev["ws"]))
+    torch.cuda.synchronize()
+    for i, (cfg, st, tree, ti, kv, dev) in enumerate(jobs):
+        ro, rl = oracle.attention(ti["q"], kv["k_cache"], kv["v_cache"], kv["kv_indptr"], None, 0, st["ctx_len"],
+                                  ti["tree_k"], ti["tree_v"], tree["mask"], tree["tree_len"])
+        v = valid_rows(tree["tree_len"], cfg.T_cap)
+        for out, lse in results[i]:
+            check_rows(out.float().cpu().numpy()[v], lse.cpu().numpy()[v], ro[v], rl[v], f"stream {i}")
 
 
 # ------------------------------------------------------------------------------------------ whole path
 
-def test_whole_path_config1(d2sd, oracle):
-    """select -> build -> attention -> accept, every stage fed by the previous one on the device."""
-    cfg = synth.CONFIGS[1]
+@pytest.mark.parametrize("cfg_no", [1, 2, 5])
+def test_whole_path(d2sd, oracle, cfg_no):
+    """select -> build -> attention (EVERY layer of the config) -> accept, every stage fed by the previous
+    one on the device, one workspace for all layers; every output of every layer against the oracle."""
+    cfg = synth.CONFIGS[cfg_no]
     st = synth.make_step_inputs(cfg)
     pl_ref, _, tree_ref = oracle_tree(oracle, cfg, st)
-    ti = synth.make_tree_inputs(cfg)
-    kv = synth.make_kv_cache(cfg, st["ctx_len"])
     logits = synth.make_logits(cfg)
     synth.plant_acceptance(cfg, logits, st["conf"], tree_ref["tokens"], tree_ref["parent"], tree_ref["depth"],
                            tree_ref["tree_len"])
     pl = d2sd.select_prefixes(torch.from_numpy(st["conf"]).cuda(), cfg.K)
-    tree = d2sd.build_tree(i32_cuda(st["draft1"]), i32_cuda(st["draft2"]), pl, i32_cuda(st["ctx_len"]), cfg.T_cap)
-    out, lse = d2sd.cascade_verify_attn(
-        bf16_cuda(ti["q"]), bf16_cuda(kv["k_cache"]), bf16_cuda(kv["v_cache"]), None, None, i32_cuda(st["ctx_len"]),
-        bf16_cuda(ti["tree_k"]), bf16_cuda(ti["tree_v"]), tree["mask"], tree["tree_len"], int(st["ctx_len"].max()))
+    ctx = i32_cuda(st["ctx_len"])
+    tree = d2sd.build_tree(i32_cuda(st["draft1"]), i32_cuda(st["draft2"]), pl, ctx, cfg.T_cap)
+    max_ctx = int(st["ctx_len"].max())
+    ws = None
+    v = valid_rows(tree_ref["tree_len"], cfg.T_cap)
+    for layer in range(cfg.layers):
+        ti = synth.make_tree_inputs(cfg, layer)
+        kv = synth.make_kv_cache(cfg, st["ctx_len"], layer)
+        kc, vc = bf16_cuda(kv["k_cache"]), bf16_cuda(kv["v_cache"])
+        if ws is None:
+            ws = d2sd.cascade_workspace(cfg.B, cfg.T_cap, cfg.Hq, cfg.Hkv, cfg.d, max_ctx, page_size=kv["page_size"],
+                                        kv_rows=kc.shape[0] * (kc.shape[1] if kv["page_size"] else 1))
+        out, lse = d2sd.cascade_verify_attn(
+            bf16_cuda(ti["q"]), kc, vc, i32_cuda(kv["kv_indptr"]),
+            None if kv["kv_indices"] is None else i32_cuda(kv["kv_indices"]), ctx, bf16_cuda(ti["tree_k"]),
+            bf16_cuda(ti["tree_v"]), tree["mask"], tree["tree_len"], max_ctx, page_size=kv["page_size"], workspace=ws)
+        torch.cuda.synchronize()
+        ro, rl = oracle.attention(ti["q"], kv["k_cache"], kv["v_cache"], kv["kv_indptr"], kv["kv_indices"],
+                                  kv["page_size"], st["ctx_len"], ti["tree_k"], ti["tree_v"], tree_ref["mask"],
+                                  tree_ref["tree_len"])
+        check_rows(out.float().cpu().numpy()[v], lse.cpu().numpy()[v], ro[v], rl[v], f"cfg{cfg_no} layer {layer}")
     acc = d2sd.accept(bf16_cuda(logits), tree["tokens"], tree["parent"], tree["depth"], tree["tree_len"], cfg.gamma)
     torch.cuda.synchronize()
-    ro, rl = oracle.attention(ti["q"], kv["k_cache"], kv["v_cache"], kv["kv_indptr"], None, 0, st["ctx_len"],
-                              ti["tree_k"], ti["tree_v"], tree_ref["mask"], tree_ref["tree_len"])
-    T = int(tree_ref["tree_len"][0])
-    check_rows(out.float().cpu().numpy()[0, :T], lse.cpu().numpy()[0, :T], ro[0, :T], rl[0, :T], "whole path")
+    assert np.array_equal(pl.cpu().numpy(), pl_ref)
+    for name in ("tokens", "parent", "depth", "pos_id", "branch_off", "tree_len"):
+        assert np.array_equal(tree[name].cpu().numpy(), tree_ref[name]), name
+    assert np.array_equal(tree["mask"].cpu().numpy().view(np.uint32), tree_ref["mask"])
     ref = oracle.accept(logits, tree_ref["tokens"], tree_ref["parent"], tree_ref["depth"], tree_ref["tree_len"], cfg.gamma)
     for name in ("argmax", "accept_len", "bonus", "best_node", "path"):
         assert np.array_equal(acc[name].cpu().numpy(), ref[name]), name

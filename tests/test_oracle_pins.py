@@ -42,11 +42,23 @@ def test_golden_paper_shapes(oracle):
         conf = np.linspace(0.9, 0.1, gamma, dtype=np.float32)[None]
         pl, r = oracle.select_prefixes(conf, K)
         if name == "n_prefix_candidates":
-            assert r.shape[1] == value
-        elif name == "n_candidates":
+            # Fig. 2b (:115): K of the `value` candidate prefix lengths {0..gamma-2} are selected, all distinct and
+            # in range, and the tree then holds gamma + sum_{i in S} (gamma-1-i) tokens (:107)
+            assert len(set(pl[0].tolist())) == K and K < value
+            assert set(pl[0].tolist()) <= set(range(value))
             tree = oracle.build_tree(np.zeros((1, gamma), np.int32), np.zeros((1, K, gamma), np.int32),
                                      pl, np.zeros(1, np.int32), synth.t_cap(gamma, K))
-            assert tree["branch_off"].shape[1] - 1 + 1 == value  # K branches + the draft-1 block
+            assert int(tree["tree_len"][0]) == gamma + sum(gamma - 1 - int(i) for i in pl[0])
+        elif name == "n_candidates":
+            # "the K+1 candidates" (:124): the flattened tree has exactly K+1 root-to-leaf paths, each of them a
+            # full block of gamma positions (every candidate runs to the block end, :107)
+            tree = oracle.build_tree(np.zeros((1, gamma), np.int32), np.zeros((1, K, gamma), np.int32),
+                                     pl, np.zeros(1, np.int32), synth.t_cap(gamma, K))
+            T = int(tree["tree_len"][0])
+            par = tree["parent"][0, :T]
+            leaves = sorted(set(range(T)) - set(par.tolist()))
+            assert len(leaves) == value
+            assert all(int(tree["depth"][0, n]) == gamma - 1 for n in leaves)
         elif name.startswith("redraft_len_i"):
             i = int(name[len("redraft_len_i"):])
             pl = np.array([[i]], np.int32)
