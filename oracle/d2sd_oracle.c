@@ -295,6 +295,120 @@ void d2sd_oracle_accept_walk(const int32_t* argmax, const int32_t* tokens, const
     free(ok);
 }
 
+/* ------------------------------------------------------------------------------------------
+ * Next row f3: confidence extraction (the step that feeds stage (a)).
+ * PAPER.md:87-89 Eq. 3: the drafter emits a categorical p_k(.) at block positions k = 1..gamma-1;
+ * t_k = argmax_v p_k(v) (greedy sample), c_k = p_k(t_k) = max_v p_k(v).
+ * p_k = softmax of the drafter's logits row (temperature 1) [G23]; argmax ties -> smallest v, IEEE
+ * comparison as in stage (d) [G18].  fp64: m = max x, s = sum_v e^(x_v - m) in index order,
+ * c = e^(x_t - m) / s = 1 / s.
+ * logits bf16 bits [B, gamma-1, V] (row r of request b at logits + (b*(gamma-1) + r)*row_stride holds
+ * block position k = r+1); anchor int32 [B].  Outputs in the layout stages (a)/(b) consume [G9]:
+ * draft [B,gamma] with draft[.,0] = anchor, conf [B,gamma] with conf[.,0] = 1.
+ * ------------------------------------------------------------------------------------------ */
+void d2sd_oracle_confidence(const uint16_t* logits, int64_t row_stride, int32_t V, const int32_t* anchor,
+                            int32_t B, int32_t gamma, int32_t* draft, double* conf) {
+    int64_t total = (int64_t)B * gamma;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t i = 0; i < total; ++i) {
+        int32_t b = (int32_t)(i / gamma), k = (int32_t)(i % gamma);
+        if (k == 0) { draft[i] = anchor[b]; conf[i] = 1.0; continue; }
+        const uint16_t* row = logits + ((size_t)b * (gamma - 1) + (size_t)(k - 1)) * row_stride;
+        int32_t best = 0;
+        double m = bf16_to_f64(row[0]);
+        for (int32_t v = 1; v < V; ++v) {
+            double x = bf16_to_f64(row[v]);
+            if (x > m) { m = x; best = v; }
+        }
+        double s = 0.0;
+        for (int32_t v = 0; v < V; ++v) s += exp(bf16_to_f64(row[v]) - m);
+        draft[i] = best;
+        conf[i] = 1.0 / s;
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Next row f1: commit of the accepted path into the KV cache (the step after stage (d)).
+ * PAPER.md:124 "commit the longest accepted prefix"; :119 each cycle "consumes the verified KV caches
+ * ... and emits a new batch of accepted tokens"; :69 "refreshed target hidden features that seed the
+ * next cycle".
+ * The verify pass computed K/V of every tree node; the nodes of path[0..accept_len] (root = anchor,
+ * then the accepted draft tokens [G10, G19]) become committed context: for j = 0..accept_len the
+ * cache row at position L + j receives the tree row of node path[j], in every layer, and the context
+ * grows by n = accept_len + 1 [G24].  The bonus token is the NEXT cycle's anchor; its K/V does not
+ * exist yet.
+ * Addressing as in stage (c).  Capacity [G25]: contiguous: request b owns rows
+ * kv_indptr[b]..kv_indptr[b+1] (kv_indptr NULL: kv_rows rows); paged: its page-table segment
+ * kv_indices[kv_indptr[b]..kv_indptr[b+1]) has ceil(L/page) pages in use; with a free list
+ * (free_pages != NULL) the next entries are filled from free_pages[*free_head ..) in request order
+ * b = 0,1,.. as far as the list lasts, without one the remaining entries are taken as already
+ * reserved by the caller.  Rows that do not fit are dropped from the END of the path:
+ * n_fit <= n, ctx_len_out = L + n_fit, dropped[b] = n - n_fit (0 = everything committed).
+ * tree_k/tree_v [n_layers][B][T_cap][Hkv][d] with element stride tree_layer_stride between layers;
+ * caches with element stride cache_layer_stride between layers.  Plain loops, byte-exact copy.
+ * ------------------------------------------------------------------------------------------ */
+void d2sd_oracle_commit_kv(const uint16_t* tree_k, const uint16_t* tree_v, int64_t tree_layer_stride,
+                           const int32_t* path, const int32_t* accept_len, const int32_t* ctx_len,
+                           uint16_t* k_cache, uint16_t* v_cache, int64_t cache_layer_stride,
+                           int64_t kv_rows, const int32_t* kv_indptr, int32_t* kv_indices,
+                           int32_t page_size, const int32_t* free_pages, int32_t n_free,
+                           int32_t* free_head, int32_t B, int32_t gamma, int32_t T_cap, int32_t Hkv,
+                           int32_t d, int32_t n_layers, int32_t* ctx_len_out, int32_t* dropped) {
+    size_t row_elems = (size_t)Hkv * d;
+    for (int32_t b = 0; b < B; ++b) {
+        int32_t L = ctx_len[b];
+        int32_t n = accept_len[b] + 1;
+        int64_t cap_rows;
+        if (page_size > 0) cap_rows = (int64_t)(kv_indptr[b + 1] - kv_indptr[b]) * page_size;
+        else cap_rows = kv_indptr ? (int64_t)(kv_indptr[b + 1] - kv_indptr[b]) : kv_rows;
+        int32_t n_fit = n;
+        if ((int64_t)L + n_fit > cap_rows) n_fit = (int32_t)(cap_rows > L ? cap_rows - L : 0);
+        if (page_size > 0 && free_pages) {
+            int32_t owned = (L + page_size - 1) / page_size;
+            int32_t want = (L + n_fit + page_size - 1) / page_size - owned;
+            int32_t left = n_free - *free_head;
+            int32_t got = want < left ? want : (left > 0 ? left : 0);
+            for (int32_t e = 0; e < got; ++e)
+                kv_indices[(size_t)kv_indptr[b] + owned + e] = free_pages[*free_head + e];
+            *free_head += got;
+            int64_t room = (int64_t)(owned + got) * page_size - L;
+            if (n_fit > room) n_fit = (int32_t)room;
+        }
+        for (int32_t layer = 0; layer < n_layers; ++layer) {
+            for (int32_t j = 0; j < n_fit; ++j) {
+                int32_t node = path[(size_t)b * gamma + j];
+                int32_t pos = L + j;
+                size_t row;
+                if (page_size > 0)
+                    row = (size_t)kv_indices[(size_t)kv_indptr[b] + pos / page_size] * page_size + (size_t)(pos % page_size);
+                else
+                    row = (size_t)(kv_indptr ? kv_indptr[b] : 0) + (size_t)pos;
+                size_t src = (size_t)layer * tree_layer_stride + ((size_t)b * T_cap + node) * row_elems;
+                size_t dst = (size_t)layer * cache_layer_stride + row * row_elems;
+                memcpy(k_cache + dst, tree_k + src, row_elems * sizeof(uint16_t));
+                memcpy(v_cache + dst, tree_v + src, row_elems * sizeof(uint16_t));
+            }
+        }
+        ctx_len_out[b] = L + n_fit;
+        dropped[b] = n - n_fit;
+    }
+}
+
+/* Same passage (:69): the target features of the accepted path, in path order, for the next cycle's
+ * drafters.  feat bf16 bits [B,T_cap,F] -> out [B,gamma,F]: out[b,j] = feat[b,path[b,j]] for
+ * j <= accept_len[b], zero rows behind. */
+void d2sd_oracle_gather_path(const uint16_t* feat, const int32_t* path, const int32_t* accept_len,
+                             int32_t B, int32_t gamma, int32_t T_cap, int32_t F, uint16_t* out) {
+    for (int32_t b = 0; b < B; ++b)
+        for (int32_t j = 0; j < gamma; ++j) {
+            uint16_t* o = out + ((size_t)b * gamma + j) * F;
+            if (j <= accept_len[b])
+                memcpy(o, feat + ((size_t)b * T_cap + path[(size_t)b * gamma + j]) * F, (size_t)F * sizeof(uint16_t));
+            else
+                memset(o, 0, (size_t)F * sizeof(uint16_t));
+        }
+}
+
 /* Number of OpenMP threads the parallel loops above will use (reported by bench.py). */
 #ifdef _OPENMP
 #include <omp.h>

@@ -674,13 +674,14 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 const uint64_t vd = smem_desc(smem + kOffRing + vi * kKvTileBytes, kKvTileBytes / 2, 1024);
 #pragma unroll
                 for (int q = 0; q < 4; ++q) {
-                    if (2 * q < ksteps) {
-                        mbar_wait(bar(kBarPFull + 4 * s + q), par);
-                        tc_fence_after();
+                    // Every piece is awaited, also the ones past a ragged tile's end that feed no MMA: the
+                    // softmax threads still store (zero) P there, and the next Q.K^T of the slot overwrites
+                    // the same TMEM columns.
+                    mbar_wait(bar(kBarPFull + 4 * s + q), par);
+                    tc_fence_after();
 #pragma unroll
-                        for (int ks = 2 * q; ks < 2 * q + 2; ++ks)
-                            if (ks < ksteps) umma_ts(od, sd + ks * 8, vd + (uint64_t)(ks * (2048 >> 4)), kIdescPV, acc | ks);
-                    }
+                    for (int ks = 2 * q; ks < 2 * q + 2; ++ks)
+                        if (ks < ksteps) umma_ts(od, sd + ks * 8, vd + (uint64_t)(ks * (2048 >> 4)), kIdescPV, acc | ks);
                 }
                 acc = 1;
                 par ^= 1;
@@ -814,6 +815,11 @@ attn_cascade_tc_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                             D2SD_TMEM_ST32(o_addr + c0, o, 0);
                         }
                         tmem_wait_st();
+                        // The P.V of this unit accumulates into all 128 O columns as soon as ONE half has
+                        // released its first piece: both halves of these 32 rows (warps w and w + 4 take the
+                        // same decision, they see the same maxima) finish their rescale before either releases.
+                        tc_fence_before();
+                        named_bar_sync(2 + w, 64);
                         if (need) {
                             m_cur = mx;
                             l_cur *= alpha;
