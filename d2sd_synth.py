@@ -66,6 +66,12 @@ def t_cap(gamma: int, K: int) -> int:
     return gamma + K * (gamma - 1) - K * (K - 1) // 2
 
 
+def t_cap3(gamma: int, K: int) -> int:
+    """Largest depth-3 tree (third cascade level): t_cap plus, per branch, a third-level continuation
+    anchored one token into the branch's tail (gamma-2-i nodes for prefix i)."""
+    return t_cap(gamma, K) + K * (gamma - 2) - K * (K - 1) // 2
+
+
 CONFIGS: Dict[int, Config] = {
     1: Config(1, "tiny", B=1, layers=1, gamma=16, K=2, V=1024, ctx=(256, 256), paged=False),
     2: Config(2, "qwen3-8b-step", B=1, layers=36, gamma=16, K=4, V=151936, ctx=(4096, 4096), paged=False),

@@ -179,3 +179,99 @@ def accept(logits: np.ndarray, tokens, parent, depth, tree_len, gamma: int) -> d
     out = accept_walk(a, tokens, parent, depth, tree_len, gamma)
     out["argmax"] = a
     return out
+
+
+# ------------------------------------------------------------------------------- next rows
+
+def confidence(logits: np.ndarray, anchor: np.ndarray):
+    """f3, Eq. 3.  logits bf16 bits [B,gamma-1,V], anchor int32 [B] ->
+    (draft int32 [B,gamma], conf fp64 [B,gamma]); slot 0 = (anchor, 1)."""
+    logits = _c(logits, np.uint16)
+    B, gm1, V = logits.shape
+    gamma = gm1 + 1
+    anchor = _c(anchor, np.int32)
+    draft = np.zeros((B, gamma), np.int32)
+    conf = np.zeros((B, gamma), np.float64)
+    _load().d2sd_oracle_confidence(_p(logits), ctypes.c_int64(V), ctypes.c_int32(V), _p(anchor),
+                                   ctypes.c_int32(B), ctypes.c_int32(gamma), _p(draft), _p(conf))
+    return draft, conf
+
+
+def commit_kv(tree_k, tree_v, path, accept_len, ctx_len, k_cache, v_cache, kv_indptr, kv_indices,
+              page_size: int, free_pages=None, free_head: int = 0):
+    """f1.  tree_k/tree_v bf16 bits [n_layers,B,T_cap,Hkv,d]; caches
+    [n_layers,rows,Hkv,d] (paged: rows = pages*page_size).  Returns a dict with the NEW k_cache,
+    v_cache, kv_indices (copies; inputs untouched), ctx_len, dropped, free_head."""
+    tree_k, tree_v = _c(tree_k, np.uint16), _c(tree_v, np.uint16)
+    n_layers, B, T_cap, Hkv, d = tree_k.shape
+    k_cache, v_cache = _c(k_cache, np.uint16).copy(), _c(v_cache, np.uint16).copy()
+    assert k_cache.shape[0] == n_layers and k_cache.shape[2:] == (Hkv, d)
+    kv_rows = k_cache.shape[1]
+    path = _c(path, np.int32)
+    gamma = path.shape[1]
+    accept_len, ctx_len = _c(accept_len, np.int32), _c(ctx_len, np.int32)
+    kv_indptr = None if kv_indptr is None else _c(kv_indptr, np.int32)
+    kv_indices = None if kv_indices is None else _c(kv_indices, np.int32).copy()
+    free_pages = None if free_pages is None else _c(free_pages, np.int32)
+    head = np.array([free_head], np.int32)
+    ctx_out = np.zeros((B,), np.int32)
+    dropped = np.zeros((B,), np.int32)
+    _load().d2sd_oracle_commit_kv(
+        _p(tree_k), _p(tree_v), ctypes.c_int64(B * T_cap * Hkv * d), _p(path), _p(accept_len), _p(ctx_len),
+        _p(k_cache), _p(v_cache), ctypes.c_int64(kv_rows * Hkv * d), ctypes.c_int64(kv_rows), _p(kv_indptr),
+        _p(kv_indices), ctypes.c_int32(page_size), _p(free_pages),
+        ctypes.c_int32(0 if free_pages is None else free_pages.size), _p(head), ctypes.c_int32(B),
+        ctypes.c_int32(gamma), ctypes.c_int32(T_cap), ctypes.c_int32(Hkv), ctypes.c_int32(d),
+        ctypes.c_int32(n_layers), _p(ctx_out), _p(dropped))
+    return {"k_cache": k_cache, "v_cache": v_cache, "kv_indices": kv_indices, "ctx_len": ctx_out,
+            "dropped": dropped, "free_head": int(head[0])}
+
+
+def gather_path(feat, path, accept_len):
+    """f1.  feat bf16 bits [B,T_cap,F] -> [B,gamma,F] rows of the accepted path, zero padded."""
+    feat = _c(feat, np.uint16)
+    B, T_cap, F = feat.shape
+    path = _c(path, np.int32)
+    gamma = path.shape[1]
+    out = np.zeros((B, gamma, F), np.uint16)
+    _load().d2sd_oracle_gather_path(_p(feat), _p(path), _p(_c(accept_len, np.int32)), ctypes.c_int32(B),
+                                    ctypes.c_int32(gamma), ctypes.c_int32(T_cap), ctypes.c_int32(F), _p(out))
+    return out
+
+
+def select_third(conf2, prefix_len):
+    """f2.  conf2 fp32 [B,K,gamma], prefix_len [B,K] -> (third_len int32 [B,K] (-1 = none),
+    r3 fp64 [B,K,gamma-1])."""
+    conf2 = _c(conf2, np.float32)
+    B, K, gamma = conf2.shape
+    prefix_len = _c(prefix_len, np.int32).reshape(B, K)
+    third = np.zeros((B, K), np.int32)
+    r3 = np.zeros((B, K, gamma - 1), np.float64)
+    _load().d2sd_oracle_select_third(_p(conf2), _p(prefix_len), ctypes.c_int32(B), ctypes.c_int32(gamma),
+                                     ctypes.c_int32(K), _p(third), _p(r3))
+    return third, r3
+
+
+def build_tree3(draft1, draft2, draft3, prefix_len, third_len, ctx_len, T_cap: int) -> dict:
+    """f2: the depth-3 tree (two-level tree + third-level continuations); branch_off [B,2K+1]."""
+    draft1 = _c(draft1, np.int32)
+    B, gamma = draft1.shape
+    prefix_len = _c(prefix_len, np.int32).reshape(B, -1)
+    K = prefix_len.shape[1]
+    draft2 = _c(draft2, np.int32).reshape(B, K, gamma)
+    draft3 = _c(draft3, np.int32).reshape(B, K, gamma)
+    third_len = _c(third_len, np.int32).reshape(B, K)
+    ctx_len = _c(ctx_len, np.int32)
+    W = (T_cap + 31) // 32
+    out = {
+        "tokens": np.zeros((B, T_cap), np.int32), "parent": np.zeros((B, T_cap), np.int32),
+        "depth": np.zeros((B, T_cap), np.int32), "pos_id": np.zeros((B, T_cap), np.int32),
+        "branch_off": np.zeros((B, 2 * K + 1), np.int32), "mask": np.zeros((B, T_cap, W), np.uint32),
+        "tree_len": np.zeros((B,), np.int32),
+    }
+    _load().d2sd_oracle_build_tree3(_p(draft1), _p(draft2), _p(draft3), _p(prefix_len), _p(third_len),
+                                    _p(ctx_len), ctypes.c_int32(B), ctypes.c_int32(gamma), ctypes.c_int32(K),
+                                    ctypes.c_int32(T_cap), _p(out["tokens"]), _p(out["parent"]),
+                                    _p(out["depth"]), _p(out["pos_id"]), _p(out["branch_off"]),
+                                    _p(out["mask"]), _p(out["tree_len"]))
+    return out

@@ -17,6 +17,9 @@
  *   build  : P3 brute force over the K+1 flat candidate sequences, P4 structural invariants
  *   attn   : P3 (flat-sequence causal attention), P5 merge invariant, P6 torch SDPA fp64 special case
  *   accept : P7 special cases, P8 per-candidate linear rule, P9 numpy.argmax + planted ties
+ *   next rows: confidence -> P10 torch.softmax fp64 + closed forms; commit_kv -> P11 two-cycle invariant
+ *   (attention over the committed cache == attention over prefix + accepted path) + brute-force
+ *   page walk; select_third / build_tree3 -> P12 exact-rational ranking, flat 2K+1 candidates, T formula
  * Parity unpinned: none of the functions below.  (alpha / speedup tables of the paper are not
  * computed here at all: they need weights and datasets.)
  */
@@ -407,6 +410,108 @@ void d2sd_oracle_gather_path(const uint16_t* feat, const int32_t* path, const in
             else
                 memset(o, 0, (size_t)F * sizeof(uint16_t));
         }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Next row f2: third cascade level (Ablation 3, Table 7).
+ * "for every i in S, we re-apply the rejection-boundary estimator (Eq. 4) to that branch's
+ * second-draft tail, take the single top-1 location j_i, and dispatch a third VP-Drafter forward
+ * anchored there.  This yields up to 2K+1 shared-prefix candidates".
+ * Branch b (prefix i_b) re-drafted block positions i_b+1..gamma-1 with confidences conf2[b][p].
+ * Eq. 4 on the tail: keeping the first j' tail tokens and losing the next one has posterior
+ *   r_b(j') = (prod_{k=1..j'} conf2[b][i_b+k]) * (1 - conf2[b][i_b+j'+1]).
+ * Reading [G22]: a third-level prefix strictly extends its branch's prefix and leaves at least one
+ * position to re-draft, j' in {1..n_b-1} with n_b = gamma-1-i_b, so the third-level prefix length
+ * in block terms j_b = i_b + j' lies in {1..gamma-2} (the set :228 names) and a branch with
+ * n_b = 1 has no third-level child ("up to" 2K+1).  Top-1, ties -> smaller j' [G5]; same fp64
+ * operation order as stage (a) [G7].
+ * conf2 fp32 [B,K,gamma]; prefix_len [B,K] -> third_len int32 [B,K] (block prefix length j_b, or
+ * -1: no child); r3_out optional fp64 [B,K,gamma-1], entry j' (0 where j' is outside the domain).
+ * ------------------------------------------------------------------------------------------ */
+void d2sd_oracle_select_third(const float* conf2, const int32_t* prefix_len, int32_t B, int32_t gamma,
+                              int32_t K, int32_t* third_len, double* r3_out) {
+    for (int32_t b = 0; b < B; ++b)
+        for (int32_t k = 0; k < K; ++k) {
+            const float* c = conf2 + ((size_t)b * K + k) * gamma;
+            int32_t i = prefix_len[(size_t)b * K + k];
+            int32_t nb = gamma - 1 - i;
+            double* r3 = r3_out ? r3_out + ((size_t)b * K + k) * (gamma - 1) : NULL;
+            if (r3) for (int32_t j = 0; j < gamma - 1; ++j) r3[j] = 0.0;
+            int32_t best = -1;
+            double best_r = 0.0;
+            volatile double P = 1.0;
+            for (int32_t j = 0; j <= nb - 1; ++j) { /* j tail tokens kept, tail token j+1 rejected */
+                volatile double one_minus = 1.0 - (double)c[i + j + 1];
+                volatile double rj = P * one_minus;
+                if (j >= 1) {
+                    if (r3) r3[j] = rj;
+                    if (best < 0 || rj > best_r) { best = j; best_r = rj; } /* strict: ties keep smaller j */
+                }
+                volatile double Pn = P * (double)c[i + j + 1];
+                P = Pn;
+            }
+            third_len[(size_t)b * K + k] = best < 0 ? -1 : i + best;
+        }
+}
+
+/* Depth-3 tree: the two-level tree of stage (b) followed, in branch order, by the third-level
+ * continuations.  Child of branch k with third_len j (>= i_k + 1): nodes for block positions
+ * p = j+1..gamma-1 with tokens draft3[k][p]; the first hangs under branch k's node at position j
+ * (node boff[k] + j - i_k - 1), the rest form a chain.  branch_off has 2K+1 entries + the end:
+ * [0..K) second-level starts, [K..2K) third-level starts (== next start when absent), [2K] = tree_len.
+ * Everything else (pos_id, mask by parent chasing, padding) as d2sd_oracle_build_tree. */
+void d2sd_oracle_build_tree3(const int32_t* draft1, const int32_t* draft2, const int32_t* draft3,
+                             const int32_t* prefix_len, const int32_t* third_len, const int32_t* ctx_len,
+                             int32_t B, int32_t gamma, int32_t K, int32_t T_cap, int32_t* tokens,
+                             int32_t* parent, int32_t* depth, int32_t* pos_id, int32_t* branch_off,
+                             uint32_t* mask, int32_t* tree_len) {
+    int32_t W = (T_cap + 31) / 32;
+    for (int32_t b = 0; b < B; ++b) {
+        int32_t* tok = tokens + (size_t)b * T_cap;
+        int32_t* par = parent + (size_t)b * T_cap;
+        int32_t* dep = depth + (size_t)b * T_cap;
+        int32_t* pos = pos_id + (size_t)b * T_cap;
+        uint32_t* mk = mask + (size_t)b * T_cap * W;
+        int32_t* boff = branch_off + (size_t)b * (2 * K + 1);
+        for (int32_t n = 0; n < T_cap; ++n) { tok[n] = -1; par[n] = -1; dep[n] = 0; pos[n] = 0; }
+        memset(mk, 0, sizeof(uint32_t) * (size_t)T_cap * W);
+        for (int32_t j = 0; j < gamma; ++j) {
+            tok[j] = draft1[(size_t)b * gamma + j];
+            par[j] = j - 1;
+            dep[j] = j;
+        }
+        int32_t off = gamma;
+        for (int32_t k = 0; k < K; ++k) {
+            int32_t i = prefix_len[(size_t)b * K + k];
+            boff[k] = off;
+            for (int32_t p = i + 1; p <= gamma - 1; ++p) {
+                int32_t n = off + (p - i - 1);
+                tok[n] = draft2[((size_t)b * K + k) * gamma + p];
+                par[n] = (p == i + 1) ? i : n - 1;
+                dep[n] = p;
+            }
+            off += gamma - 1 - i;
+        }
+        for (int32_t k = 0; k < K; ++k) {
+            int32_t i = prefix_len[(size_t)b * K + k];
+            int32_t j = third_len[(size_t)b * K + k];
+            boff[K + k] = off;
+            if (j < 0) continue;
+            for (int32_t p = j + 1; p <= gamma - 1; ++p) {
+                int32_t n = off + (p - j - 1);
+                tok[n] = draft3[((size_t)b * K + k) * gamma + p];
+                par[n] = (p == j + 1) ? boff[k] + (j - i - 1) : n - 1;
+                dep[n] = p;
+            }
+            off += gamma - 1 - j;
+        }
+        boff[2 * K] = off;
+        tree_len[b] = off;
+        for (int32_t n = 0; n < off; ++n) {
+            pos[n] = ctx_len[b] + dep[n];
+            for (int32_t a = n; a >= 0; a = par[a]) mk[(size_t)n * W + a / 32] |= (1u << (a % 32));
+        }
+    }
 }
 
 /* Number of OpenMP threads the parallel loops above will use (reported by bench.py). */
