@@ -195,6 +195,107 @@ int32_t d2sd_accept(const void* logits, int64_t row_stride, int32_t V, const int
                     int32_t* path, int32_t* bonus, int32_t* best_node, void* workspace,
                     size_t workspace_bytes, void* stream);
 
+/* =============================================================================================
+ * The steps around the hot path (SURVEY.md 8f "next" rows), same conventions as above.
+ * ============================================================================================= */
+
+/* ---------------------------------------------------------------------------------------------
+ * Confidence extraction, the step BEFORE (a).  PAPER.md:87-89, Eq. 3: the drafter emits a
+ * categorical p_k(.) at block positions k = 1..gamma-1; t_k = argmax_v p_k(v) (greedy sample) and
+ * c_k = p_k(t_k) = max_v p_k(v).  p_k = softmax of the logits row (temperature 1), so
+ * c_k = 1 / sum_v exp(x_v - max_v x).  One vocabulary pass per row: (max, first index of the max,
+ * sum of exponentials) per 16384-entry chunk, merged by a second small kernel.
+ *   logits      bf16, drafter row of block position k (1..gamma-1) of request b at
+ *               logits + (b*(gamma-1) + k-1)*row_stride elements, V entries
+ *   anchor      int32 [B], the bonus token of the previous cycle (:69)
+ *   draft       out int32 [B,gamma]: draft[b,0] = anchor[b], draft[b,k] = t_k (ties -> smallest v)
+ *   conf        out fp32 [B,gamma]: conf[b,0] = 1, conf[b,k] = c_k -- the layout (a) and (b) consume
+ *   workspace   >= d2sd_confidence_workspace_bytes(B,gamma,V) bytes, 16-byte aligned; scratch
+ * Arithmetic: fp32 sums of ex2.approx exponentials; c_k agrees with the fp64 definition to ~1e-6
+ * relative (tests gate 2e-5); t_k is bit-exact.  Requires 2 <= gamma <= 64, V >= 1, row_stride >= V.
+ * ------------------------------------------------------------------------------------------- */
+size_t d2sd_confidence_workspace_bytes(int32_t B, int32_t gamma, int32_t V);
+
+int32_t d2sd_draft_confidence(const void* logits, int64_t row_stride, int32_t V, const int32_t* anchor,
+                              int32_t B, int32_t gamma, int32_t* draft, float* conf, void* workspace,
+                              size_t workspace_bytes, void* stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * KV commit, the step AFTER (d).  PAPER.md:124 "commit the longest accepted prefix"; :119 each cycle
+ * "consumes the verified KV caches ... and emits a new batch of accepted tokens"; :69 "refreshed
+ * target hidden features that seed the next cycle".
+ * The verify pass computed K/V of every tree node.  For j = 0..accept_len[b] the cache row at
+ * position ctx_len[b] + j of EVERY layer receives the tree row of node path[b,j] (path[b,0] is the
+ * root = this cycle's anchor, whose K/V the target had not seen before); the context grows by
+ * accept_len[b] + 1.  The bonus token is the next cycle's anchor and has no K/V yet.
+ *   tree_k, tree_v   bf16 [n_layers][B,T_cap,Hkv,d], layer l at + l*tree_layer_stride elements
+ *   path, accept_len int32 [B,gamma] / [B] as written by d2sd_accept
+ *   ctx_len          int32 [B] committed length before the call
+ *   k_cache, v_cache bf16, in/out; layer l at + l*cache_layer_stride elements; addressing as in (c)
+ *   kv_indptr        int32 [B+1]: contiguous: request b owns rows kv_indptr[b] .. kv_indptr[b+1]-1 of
+ *                    which ctx_len[b] are in use (NULL iff B == 1: rows 0 .. kv_rows-1); paged: its
+ *                    page-table segment kv_indices[kv_indptr[b] .. kv_indptr[b+1]) of which
+ *                    ceil(ctx_len[b]/page_size) entries are in use
+ *   kv_indices       paged: int32, in/out when a free list is given; contiguous: NULL
+ *   free_pages, n_free, free_head   optional free list (NULL, 0, NULL: the unused entries of each
+ *                    segment are already valid pages, reserved by the caller).  With a list, the pages a
+ *                    request newly needs are taken from free_pages[*free_head ..) in request order
+ *                    b = 0,1,.., written into its segment, and *free_head advances (device int32).
+ *   ctx_len_out      out int32 [B] = ctx_len + rows committed; MAY alias ctx_len
+ *   dropped          out int32 [B]: rows that did not fit (segment full / free list exhausted), cut
+ *                    from the END of the path; 0 = everything committed
+ *   feat, feat_out   optional (both or neither): bf16 [B,T_cap,F] target features of every node ->
+ *                    [B,gamma,F], feat_out[b,j] = feat[b,path[b,j]] for j <= accept_len[b], zero rows behind
+ *   workspace        >= d2sd_commit_workspace_bytes(B) bytes, 16-byte aligned; scratch
+ * Byte-exact copies.  Requires (Hkv*d) % 8 == 0, F % 8 == 0, 16-byte aligned tensors and layer strides,
+ * page_size 0 or > 0 (any), B <= 65535, n_layers <= 65535.
+ * ------------------------------------------------------------------------------------------- */
+typedef struct d2sd_commit_params {
+    int32_t B, gamma, T_cap, Hkv, d, n_layers;
+    int32_t page_size;          /* 0 = contiguous */
+    int64_t kv_rows;            /* token rows per layer of k_cache / v_cache */
+    int64_t tree_layer_stride;  /* elements between layers of tree_k / tree_v (>= B*T_cap*Hkv*d) */
+    int64_t cache_layer_stride; /* elements between layers of the caches (>= kv_rows*Hkv*d) */
+    int32_t F;                  /* feature width, 0 without feat */
+} d2sd_commit_params;
+
+size_t d2sd_commit_workspace_bytes(int32_t B);
+
+int32_t d2sd_commit_kv(const d2sd_commit_params* p /* host */, const void* tree_k, const void* tree_v,
+                       const int32_t* path, const int32_t* accept_len, const int32_t* ctx_len, void* k_cache,
+                       void* v_cache, const int32_t* kv_indptr, int32_t* kv_indices, const int32_t* free_pages,
+                       int32_t n_free, int32_t* free_head, int32_t* ctx_len_out, int32_t* dropped,
+                       const void* feat, void* feat_out, void* workspace, size_t workspace_bytes, void* stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * Third cascade level.  PAPER.md:228-240 (Ablation 3, Table 7): "for every i in S, we re-apply the
+ * rejection-boundary estimator (Eq. 4) to that branch's second-draft tail, take the single top-1
+ * location j_i, and dispatch a third VP-Drafter forward anchored there.  This yields up to 2K+1
+ * shared-prefix candidates that the target jointly verifies in a single pass".
+ * d2sd_select_third: branch k (prefix i_k) re-drafted positions i_k+1..gamma-1 with confidences
+ * conf2[b,k,p].  r_k(j') = (prod_{m=1..j'} conf2[i_k+m]) * (1 - conf2[i_k+j'+1]) for j' = 1..n_k-1,
+ * n_k = gamma-1-i_k (the third-level prefix strictly extends the branch's and leaves a position to
+ * re-draft, so its block prefix length i_k+j' is in {1..gamma-2}, :228); top-1, ties -> smaller j';
+ * same fp64 operation order as (a).
+ *   conf2       fp32 [B,K,gamma];  prefix_len int32 [B,K] from (a)
+ *   third_len   out int32 [B,K]: block prefix length j_k in [i_k+1, gamma-2], or -1 (n_k = 1: no child)
+ *   r3_out      out fp64 [B,K,gamma-1] (entry j'; 0 outside the domain), or NULL
+ * d2sd_build_tree3: the tree of d2sd_build_tree followed, in branch order, by the third-level
+ * continuations: child of branch k holds draft3[b,k,j_k+1..gamma-1]; its first node's parent is branch
+ * k's node at block position j_k.  branch_off out [B,2K+1]: [0..K) second-level starts, [K..2K)
+ * third-level starts (an absent child: the next start), [2K] = tree_len.  T_cap must hold the largest
+ * depth-3 tree: gamma + K(gamma-1) - K(K-1)/2 + K(gamma-2) - K(K-1)/2.  Everything else as (b); the
+ * result feeds d2sd_cascade_verify_attn and d2sd_accept unchanged.
+ * ------------------------------------------------------------------------------------------- */
+int32_t d2sd_select_third(const float* conf2, const int32_t* prefix_len, int32_t B, int32_t gamma, int32_t K,
+                          int32_t* third_len, double* r3_out, void* stream);
+
+int32_t d2sd_build_tree3(const int32_t* draft1, const int32_t* draft2, const int32_t* draft3,
+                         const int32_t* prefix_len, const int32_t* third_len, const int32_t* ctx_len, int32_t B,
+                         int32_t gamma, int32_t K, int32_t T_cap, int32_t* tokens, int32_t* parent,
+                         int32_t* depth, int32_t* pos_id, int32_t* branch_off, uint32_t* mask,
+                         int32_t* tree_len, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

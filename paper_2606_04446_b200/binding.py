@@ -1,4 +1,4 @@
-"""ctypes binding of libd2sd.so: the four calls of include/d2sd.h with torch tensors as buffers.
+"""ctypes binding of libd2sd.so: the calls of include/d2sd.h with torch tensors as buffers.
 
 Argument marshalling only -- every step of the path runs in the library's CUDA kernels.  Output
 tensors are allocated here with torch (device memory is PyTorch's job) unless the caller passes
@@ -32,6 +32,14 @@ class _AttnParams(ctypes.Structure):
                 ("phases", ctypes.c_int32)]
 
 
+class _CommitParams(ctypes.Structure):
+    _fields_ = [("B", ctypes.c_int32), ("gamma", ctypes.c_int32), ("T_cap", ctypes.c_int32),
+                ("Hkv", ctypes.c_int32), ("d", ctypes.c_int32), ("n_layers", ctypes.c_int32),
+                ("page_size", ctypes.c_int32), ("kv_rows", ctypes.c_int64),
+                ("tree_layer_stride", ctypes.c_int64), ("cache_layer_stride", ctypes.c_int64),
+                ("F", ctypes.c_int32)]
+
+
 def lib_path() -> str:
     return _LIB_PATH
 
@@ -62,6 +70,19 @@ def lib() -> ctypes.CDLL:
         L.d2sd_accept.restype = i32
         L.d2sd_accept.argtypes = [vp, i64, i32, vp, vp, vp, vp, i32, i32, i32, vp, vp, vp, vp, vp, vp,
                                   ctypes.c_size_t, vp]
+        L.d2sd_confidence_workspace_bytes.restype = ctypes.c_size_t
+        L.d2sd_confidence_workspace_bytes.argtypes = [i32, i32, i32]
+        L.d2sd_draft_confidence.restype = i32
+        L.d2sd_draft_confidence.argtypes = [vp, i64, i32, vp, i32, i32, vp, vp, vp, ctypes.c_size_t, vp]
+        L.d2sd_commit_workspace_bytes.restype = ctypes.c_size_t
+        L.d2sd_commit_workspace_bytes.argtypes = [i32]
+        L.d2sd_commit_kv.restype = i32
+        L.d2sd_commit_kv.argtypes = ([ctypes.POINTER(_CommitParams)] + [vp] * 10 + [i32] + [vp] * 6 +
+                                     [ctypes.c_size_t, vp])
+        L.d2sd_select_third.restype = i32
+        L.d2sd_select_third.argtypes = [vp, vp, i32, i32, i32, vp, vp, vp]
+        L.d2sd_build_tree3.restype = i32
+        L.d2sd_build_tree3.argtypes = [vp] * 6 + [i32] * 4 + [vp] * 8
         _lib = L
     return _lib
 
@@ -254,4 +275,109 @@ def accept(logits: torch.Tensor, tokens: torch.Tensor, parent: torch.Tensor, dep
                              _ptr(tree_len), B, gamma, T_cap, _ptr(out["argmax"]), _ptr(out["accept_len"]),
                              _ptr(out["path"]), _ptr(out["bonus"]), _ptr(out["best_node"]), _ptr(workspace),
                              workspace.numel() * workspace.element_size(), _stream()))
+    return out
+
+
+# ------------------------------------------------------------------------- the steps around the path
+
+def t_cap3(gamma: int, K: int) -> int:
+    """Largest depth-3 tree (include/d2sd.h, d2sd_build_tree3)."""
+    return t_cap(gamma, K) + K * (gamma - 2) - K * (K - 1) // 2
+
+
+def confidence_workspace_bytes(B: int, gamma: int, V: int) -> int:
+    return int(lib().d2sd_confidence_workspace_bytes(B, gamma, V))
+
+
+def draft_confidence(logits: torch.Tensor, anchor: torch.Tensor, draft: Optional[torch.Tensor] = None,
+                     conf: Optional[torch.Tensor] = None, workspace: Optional[torch.Tensor] = None):
+    """d2sd_draft_confidence: drafter logits bf16 [B,gamma-1,V], anchor int32 [B] ->
+    (draft int32 [B,gamma], conf fp32 [B,gamma]), slot 0 = (anchor, 1)."""
+    if not (logits.is_cuda and logits.dtype == torch.bfloat16 and logits.dim() == 3 and logits.stride(2) == 1
+            and logits.stride(0) == logits.shape[1] * logits.stride(1)):
+        raise TypeError("logits: expected CUDA bf16 [B,gamma-1,V] with unit inner stride and uniform row stride")
+    B, gm1, V = logits.shape
+    gamma = gm1 + 1
+    _dev(anchor, torch.int32, "anchor")
+    draft = _out(draft, (B, gamma), torch.int32, logits.device, "draft")
+    conf = _out(conf, (B, gamma), torch.float32, logits.device, "conf")
+    if workspace is None:
+        workspace = torch.empty(confidence_workspace_bytes(B, gamma, V), dtype=torch.uint8, device=logits.device)
+    _check(lib().d2sd_draft_confidence(_ptr(logits), logits.stride(1), V, _ptr(anchor), B, gamma, _ptr(draft),
+                                       _ptr(conf), _ptr(workspace), workspace.numel(), _stream()))
+    return draft, conf
+
+
+def commit_kv(tree_k: torch.Tensor, tree_v: torch.Tensor, path: torch.Tensor, accept_len: torch.Tensor,
+              ctx_len: torch.Tensor, k_cache: torch.Tensor, v_cache: torch.Tensor,
+              kv_indptr: Optional[torch.Tensor], kv_indices: Optional[torch.Tensor], page_size: int = 0, *,
+              free_pages: Optional[torch.Tensor] = None, free_head: Optional[torch.Tensor] = None,
+              ctx_len_out: Optional[torch.Tensor] = None, dropped: Optional[torch.Tensor] = None,
+              feat: Optional[torch.Tensor] = None, feat_out: Optional[torch.Tensor] = None,
+              workspace: Optional[torch.Tensor] = None):
+    """d2sd_commit_kv.  tree_k/tree_v bf16 [n_layers,B,T_cap,Hkv,d]; caches bf16 [n_layers,rows,Hkv,d]
+    (paged: rows = pages*page_size), updated IN PLACE; returns (ctx_len_out, dropped[, feat_out])."""
+    bf = torch.bfloat16
+    for t, n in ((tree_k, "tree_k"), (tree_v, "tree_v"), (k_cache, "k_cache"), (v_cache, "v_cache")):
+        _dev(t, bf, n)
+    for t, n in ((path, "path"), (accept_len, "accept_len"), (ctx_len, "ctx_len")):
+        _dev(t, torch.int32, n)
+    n_layers, B, T_cap, Hkv, d = tree_k.shape
+    gamma = path.shape[1]
+    kv_rows = k_cache.shape[1]
+    if k_cache.shape[0] != n_layers or tuple(k_cache.shape[2:]) != (Hkv, d):
+        raise ValueError(f"k_cache: shape {tuple(k_cache.shape)} does not match [n_layers, rows, {Hkv}, {d}]")
+    dev = tree_k.device
+    ctx_len_out = _out(ctx_len_out, (B,), torch.int32, dev, "ctx_len_out")
+    dropped = _out(dropped, (B,), torch.int32, dev, "dropped")
+    F = 0
+    if feat is not None:
+        _dev(feat, bf, "feat")
+        F = feat.shape[2]
+        feat_out = _out(feat_out, (B, gamma, F), bf, dev, "feat_out")
+    p = _CommitParams(B=B, gamma=gamma, T_cap=T_cap, Hkv=Hkv, d=d, n_layers=n_layers, page_size=page_size,
+                      kv_rows=kv_rows, tree_layer_stride=B * T_cap * Hkv * d, cache_layer_stride=kv_rows * Hkv * d, F=F)
+    need = int(lib().d2sd_commit_workspace_bytes(B))
+    if workspace is None:
+        workspace = torch.empty(need, dtype=torch.uint8, device=dev)
+    _check(lib().d2sd_commit_kv(ctypes.byref(p), _ptr(tree_k), _ptr(tree_v), _ptr(path), _ptr(accept_len), _ptr(ctx_len),
+                                _ptr(k_cache), _ptr(v_cache), _ptr(kv_indptr), _ptr(kv_indices), _ptr(free_pages),
+                                0 if free_pages is None else free_pages.numel(), _ptr(free_head), _ptr(ctx_len_out),
+                                _ptr(dropped), _ptr(feat), _ptr(feat_out), _ptr(workspace), workspace.numel(), _stream()))
+    return (ctx_len_out, dropped) if feat is None else (ctx_len_out, dropped, feat_out)
+
+
+def select_third(conf2: torch.Tensor, prefix_len: torch.Tensor, third_len: Optional[torch.Tensor] = None,
+                 r3_out: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """d2sd_select_third: conf2 fp32 [B,K,gamma], prefix_len int32 [B,K] -> third_len int32 [B,K] (-1 = none)."""
+    _dev(conf2, torch.float32, "conf2")
+    _dev(prefix_len, torch.int32, "prefix_len")
+    B, K, gamma = conf2.shape
+    third_len = _out(third_len, (B, K), torch.int32, conf2.device, "third_len")
+    if r3_out is not None:
+        _out(r3_out, (B, K, gamma - 1), torch.float64, conf2.device, "r3_out")
+    _check(lib().d2sd_select_third(_ptr(conf2), _ptr(prefix_len), B, gamma, K, _ptr(third_len), _ptr(r3_out), _stream()))
+    return third_len
+
+
+def build_tree3(draft1: torch.Tensor, draft2: torch.Tensor, draft3: torch.Tensor, prefix_len: torch.Tensor,
+                third_len: torch.Tensor, ctx_len: torch.Tensor, T_cap: Optional[int] = None) -> Dict[str, torch.Tensor]:
+    """d2sd_build_tree3 -> the dict of build_tree with branch_off [B,2K+1]."""
+    B, gamma = draft1.shape
+    K = prefix_len.shape[1]
+    for t, n in ((draft1, "draft1"), (draft2, "draft2"), (draft3, "draft3"), (prefix_len, "prefix_len"),
+                 (third_len, "third_len"), (ctx_len, "ctx_len")):
+        _dev(t, torch.int32, n)
+    if T_cap is None:
+        T_cap = t_cap3(gamma, K)
+    W = (T_cap + 31) // 32
+    dev = draft1.device
+    out = {name: torch.empty((B, T_cap), dtype=torch.int32, device=dev) for name in ("tokens", "parent", "depth", "pos_id")}
+    out["branch_off"] = torch.empty((B, 2 * K + 1), dtype=torch.int32, device=dev)
+    out["mask"] = torch.empty((B, T_cap, W), dtype=torch.int32, device=dev)
+    out["tree_len"] = torch.empty((B,), dtype=torch.int32, device=dev)
+    _check(lib().d2sd_build_tree3(_ptr(draft1), _ptr(draft2), _ptr(draft3), _ptr(prefix_len), _ptr(third_len),
+                                  _ptr(ctx_len), B, gamma, K, T_cap, _ptr(out["tokens"]), _ptr(out["parent"]),
+                                  _ptr(out["depth"]), _ptr(out["pos_id"]), _ptr(out["branch_off"]), _ptr(out["mask"]),
+                                  _ptr(out["tree_len"]), _stream()))
     return out

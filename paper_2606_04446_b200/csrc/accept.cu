@@ -1,15 +1,21 @@
-// Stage (d): vocab-wide argmax + longest-accepted-path walk.  PAPER.md:69, :124.
-// Kernel 1 is a pure HBM scan (T*V bf16 values read once, 128-bit loads, no reuse -> no shared
-// memory staging, no tensor cores); kernel 2 is launch-latency-sized.
+// Vocabulary scans: stage (d) argmax + longest-accepted-path walk and the drafter
+// confidence extraction that feeds stage (a) (Eq. 3: t_k = argmax_v p_k(v), c_k = max_v p_k(v)).
+// The scan is a pure HBM stream (rows*V bf16 values read once, 128-bit loads, no reuse -> no shared
+// tensor cores): a CTA covers kScanChunk vocabulary entries of one row, brought into shared memory by
+// two 16 KiB bulk copies (cp.async.bulk, mbarrier completion, evict-first) so that 32 KiB per CTA are in
+// flight by construction; all CTAs of a launch are co-resident (4-5 per SM at config 2: ~150 KiB per SM).  The finishing kernels are
+// launch-latency-sized and start under programmatic dependent launch.
 #include <climits>
 
 #include "common.cuh"
 
 namespace d2sd {
 
-struct ArgPart {
+struct ScanPart {  // partial state of one (row, chunk): maximum, its first index, sum of e^(x - maximum)
     float v;
     int32_t i;
+    float s;
+    float pad;
 };
 
 // "x at index xi beats the current best": larger value, or equal value (IEEE: -0 == +0) at a
@@ -28,71 +34,149 @@ __device__ __forceinline__ uint4 ld_stream_16B(const void* p) {
                  : "l"(p));
     return r;
 }
+__device__ __forceinline__ float bf_lo(uint32_t w) { return __uint_as_float(w << 16); }
+__device__ __forceinline__ float bf_hi(uint32_t w) { return __uint_as_float(w & 0xFFFF0000u); }
 
 __device__ __forceinline__ void arg_update_word(uint32_t w, int idx, float& bv, int& bi) {
-    arg_update(__uint_as_float(w << 16), idx, bv, bi);
-    arg_update(__uint_as_float(w & 0xFFFF0000u), idx + 1, bv, bi);
+    arg_update(bf_lo(w), idx, bv, bi);
+    arg_update(bf_hi(w), idx + 1, bv, bi);
+}
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+__device__ __forceinline__ void scan_mbar_wait(uint32_t bar) {  // phase 0 of a one-shot barrier
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "W_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], 0;\n\t"
+        "@!p bra W_%=;\n\t}" ::"r"(bar)
+        : "memory");
 }
 
-constexpr int kArgmaxThreads = 256;
-constexpr int kArgmaxVecPerThread = kArgmaxChunk / 8 / kArgmaxThreads;  // 4 x 16 B in flight
+constexpr int kScanThreads = 256;
+constexpr int kVec = kScanChunk / 8 / kScanThreads;  // 8 x 16 B in flight per thread
+static_assert(kVec * 8 * kScanThreads == kScanChunk, "chunk = threads x vectors");
 
-// grid = (B*T_cap, chunks).  Each CTA scans kArgmaxChunk vocabulary entries of one logits row.
-__global__ void __launch_bounds__(kArgmaxThreads)
-argmax_partial_kernel(const __nv_bfloat16* __restrict__ logits, int64_t row_stride, int V,
-                      const int32_t* __restrict__ tree_len, int T_cap, int n_chunks,
-                      ArgPart* __restrict__ part) {
+// softmax-state merge of (m, i, s) pairs: first-index maximum, sums rescaled to the common maximum
+__device__ __forceinline__ void state_merge(float ov, int oi, float os, float& bv, int& bi, float& bs) {
+    const float m = fmaxf(ov, bv);
+    const float a = ov == m ? 1.f : __expf(ov - m), c = bv == m ? 1.f : __expf(bv - m);
+    bs = (os > 0.f ? os * a : 0.f) + (bs > 0.f ? bs * c : 0.f);
+    arg_update(ov, oi, bv, bi);
+}
+
+// grid = (rows, chunks).  Row r of group b = r / rows_per_group is skipped when its index inside the
+// group is >= row_limit[b] (tree padding rows; row_limit == NULL: every row is real).  kSum: also the
+// sum of e^(x - max) over the chunk (confidence extraction); otherwise argmax only.
+template <bool kSum>
+__global__ void __launch_bounds__(kScanThreads)
+vocab_scan_kernel(const __nv_bfloat16* __restrict__ logits, int64_t row_stride, int V,
+                  const int32_t* __restrict__ row_limit, int rows_per_group, int n_chunks,
+                  ScanPart* __restrict__ part) {
     const int row = blockIdx.x;
-    const int b = row / T_cap, n = row - b * T_cap;
-    if (n >= tree_len[b]) return;  // padding rows are never read
+    pdl_launch_dependents();
+    pdl_wait();  // logits and row_limit (tree_len) are written by earlier kernels of the stream
+    if (row_limit) {
+        const int b = row / rows_per_group;
+        if (row - b * rows_per_group >= row_limit[b]) return;  // padding rows are never read
+    }
     const __nv_bfloat16* rowp = logits + (size_t)row * row_stride;
-    const int start = blockIdx.y * kArgmaxChunk;
-    const int end = min(V, start + kArgmaxChunk);
-    float bv = -INFINITY;
+    const int start = blockIdx.y * kScanChunk;
+    const int end = min(V, start + kScanChunk);
+    float bv = -INFINITY, bs = 0.f;
     int bi = INT_MAX;
     const int tid = threadIdx.x;
     if ((reinterpret_cast<uintptr_t>(rowp) & 15) == 0) {
+        // The chunk is staged through shared memory by two bulk copies (one elected thread, mbarrier
+        // completion): 32 KiB per CTA are in flight whatever the compiler does with the consuming loop
+        // (ptxas interleaves plain vector loads with their compares and keeps only two in flight).
         const int nvec = (end - start) >> 3;
-        const uint4* vp = reinterpret_cast<const uint4*>(rowp + start);
-        uint4 x[kArgmaxVecPerThread];
-#pragma unroll
-        for (int u = 0; u < kArgmaxVecPerThread; ++u) {
-            const int v = tid + u * kArgmaxThreads;
-            if (v < nvec) x[u] = ld_stream_16B(vp + v);
-        }
-#pragma unroll
-        for (int u = 0; u < kArgmaxVecPerThread; ++u) {
-            const int v = tid + u * kArgmaxThreads;
-            if (v < nvec) {
-                const int idx = start + v * 8;
-                arg_update_word(x[u].x, idx, bv, bi);
-                arg_update_word(x[u].y, idx + 2, bv, bi);
-                arg_update_word(x[u].z, idx + 4, bv, bi);
-                arg_update_word(x[u].w, idx + 6, bv, bi);
+        __shared__ __align__(128) uint4 stage[kScanChunk / 8];
+        __shared__ __align__(8) unsigned long long bars[2];
+        const uint32_t bar0 = (uint32_t)__cvta_generic_to_shared(bars);
+        const uint32_t st0 = (uint32_t)__cvta_generic_to_shared(stage);
+        const int nv0 = min(nvec, kScanChunk / 16), nv1 = nvec - nv0;  // first / second half
+        if (tid == 0) {
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar0));
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar0 + 8));
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+            const char* src = reinterpret_cast<const char*>(rowp + start);
+            if (nv0 > 0) {
+                asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar0), "r"(nv0 * 16) : "memory");
+                asm volatile(
+                    "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+                    ::"r"(st0), "l"(src), "r"(nv0 * 16), "r"(bar0), "l"(0x12F0000000000000ull) : "memory");
+            }
+            if (nv1 > 0) {
+                asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar0 + 8), "r"(nv1 * 16) : "memory");
+                asm volatile(
+                    "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+                    ::"r"(st0 + nv0 * 16), "l"(src + (size_t)nv0 * 16), "r"(nv1 * 16), "r"(bar0 + 8),
+                    "l"(0x12F0000000000000ull) : "memory");
             }
         }
-        for (int i = start + nvec * 8 + tid; i < end; i += kArgmaxThreads)
-            arg_update(__bfloat162float(rowp[i]), i, bv, bi);
-    } else {
-        for (int i = start + tid; i < end; i += kArgmaxThreads)
-            arg_update(__bfloat162float(rowp[i]), i, bv, bi);
+        __syncthreads();  // barrier initialisation visible to the waiting threads
+        uint4 x[kVec];
+#pragma unroll
+        for (int u = 0; u < kVec; ++u) {
+            if (u == 0 && nv0 > 0) scan_mbar_wait(bar0);
+            if (u == kVec / 2 && nv1 > 0) scan_mbar_wait(bar0 + 8);
+            const int v = tid + u * kScanThreads;
+            x[u] = v < nvec ? stage[v] : make_uint4(0xFF80FF80u, 0xFF80FF80u, 0xFF80FF80u, 0xFF80FF80u);
+        }
+#pragma unroll
+        for (int u = 0; u < kVec; ++u) {
+            const int idx = start + (tid + u * kScanThreads) * 8;  // absent vectors hold -inf: never win
+            arg_update_word(x[u].x, idx, bv, bi);
+            arg_update_word(x[u].y, idx + 2, bv, bi);
+            arg_update_word(x[u].z, idx + 4, bv, bi);
+            arg_update_word(x[u].w, idx + 6, bv, bi);
+        }
+        const int tail0 = start + nvec * 8;  // < 8 leftover elements of the chunk
+        float xt = -INFINITY;
+        if (tail0 + tid < end) {
+            xt = __bfloat162float(rowp[tail0 + tid]);
+            arg_update(xt, tail0 + tid, bv, bi);
+        }
+        if (kSum && bv > -INFINITY) {
+#pragma unroll
+            for (int u = 0; u < kVec; ++u) {
+                const uint32_t w[4] = {x[u].x, x[u].y, x[u].z, x[u].w};
+#pragma unroll
+                for (int e = 0; e < 4; ++e) bs += __expf(bf_lo(w[e]) - bv) + __expf(bf_hi(w[e]) - bv);
+            }
+            bs += __expf(xt - bv);
+        }
+    } else {  // misaligned row start (odd strides): plain loads
+        for (int i = start + tid; i < end; i += kScanThreads) arg_update(__bfloat162float(rowp[i]), i, bv, bi);
+        if (kSum && bv > -INFINITY)
+            for (int i = start + tid; i < end; i += kScanThreads) bs += __expf(__bfloat162float(rowp[i]) - bv);
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
         const float ov = __shfl_xor_sync(0xffffffffu, bv, o);
         const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
-        arg_update(ov, oi, bv, bi);
+        if (kSum) {
+            const float os = __shfl_xor_sync(0xffffffffu, bs, o);
+            state_merge(ov, oi, os, bv, bi, bs);
+        } else {
+            arg_update(ov, oi, bv, bi);
+        }
     }
-    __shared__ float sv[kArgmaxThreads / 32];
-    __shared__ int si[kArgmaxThreads / 32];
+    __shared__ float sv[kScanThreads / 32], ss[kScanThreads / 32];
+    __shared__ int si[kScanThreads / 32];
     if ((tid & 31) == 0) {
         sv[tid >> 5] = bv;
         si[tid >> 5] = bi;
+        ss[tid >> 5] = bs;
     }
     __syncthreads();
     if (tid == 0) {
-        for (int w = 1; w < kArgmaxThreads / 32; ++w) arg_update(sv[w], si[w], bv, bi);
-        part[(size_t)row * n_chunks + blockIdx.y] = ArgPart{bv, bi};
+        for (int w = 1; w < kScanThreads / 32; ++w) {
+            if (kSum) state_merge(sv[w], si[w], ss[w], bv, bi, bs);
+            else arg_update(sv[w], si[w], bv, bi);
+        }
+        part[(size_t)row * n_chunks + blockIdx.y] = ScanPart{bv, bi, bs, 0.f};
     }
 }
 
@@ -100,7 +184,7 @@ argmax_partial_kernel(const __nv_bfloat16* __restrict__ logits, int64_t row_stri
 //   ok[n] = every edge on the path root..n has tokens[child] == a[parent]
 //   best  = deepest ok node, ties -> smallest node index.
 __global__ void __launch_bounds__(256)
-accept_walk_kernel(const ArgPart* __restrict__ part, int n_chunks, const int32_t* __restrict__ tokens,
+accept_walk_kernel(const ScanPart* __restrict__ part, int n_chunks, const int32_t* __restrict__ tokens,
                    const int32_t* __restrict__ parent, const int32_t* __restrict__ depth,
                    const int32_t* __restrict__ tree_len, int gamma, int T_cap,
                    int32_t* __restrict__ argmax_out, int32_t* __restrict__ accept_len,
@@ -112,15 +196,17 @@ accept_walk_kernel(const ArgPart* __restrict__ part, int n_chunks, const int32_t
     int32_t* tok_s = sm + 2 * T_cap;
     __shared__ int red_s[8];
     const int b = blockIdx.x;
-    const int T = tree_len[b];
     const int tid = threadIdx.x;
+    pdl_launch_dependents();
+    pdl_wait();
+    const int T = tree_len[b];
     for (int n = tid; n < T_cap; n += blockDim.x) {
         const size_t o = (size_t)b * T_cap + n;
         int a = -1;
         if (n < T) {
             float bv = -INFINITY;
             int bi = INT_MAX;
-            const ArgPart* p = part + o * n_chunks;
+            const ScanPart* p = part + o * n_chunks;
             for (int c = 0; c < n_chunks; ++c) arg_update(p[c].v, p[c].i, bv, bi);
             a = bi == INT_MAX ? 0 : bi;  // a row of NaNs only: index 0, never an out-of-range token id
             par_s[n] = parent[o];
@@ -161,21 +247,75 @@ accept_walk_kernel(const ArgPart* __restrict__ part, int n_chunks, const int32_t
     }
 }
 
+// grid = ceil(B*gamma / 128).  One thread per (request, block position): merges the chunk states of a
+// drafter row into t_k and c_k = e^(x_t - m) / sum_v e^(x_v - m) = 1 / sum (Eq. 3); slot 0 = (anchor, 1).
+__global__ void __launch_bounds__(128)
+confidence_finish_kernel(const ScanPart* __restrict__ part, int n_chunks, const int32_t* __restrict__ anchor,
+                         int B, int gamma, int32_t* __restrict__ draft, float* __restrict__ conf) {
+    pdl_launch_dependents();
+    pdl_wait();
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= B * gamma) return;
+    const int b = e / gamma, k = e - b * gamma;
+    if (k == 0) {
+        draft[e] = anchor[b];
+        conf[e] = 1.0f;
+        return;
+    }
+    const ScanPart* p = part + ((size_t)b * (gamma - 1) + (k - 1)) * n_chunks;
+    float bv = -INFINITY, bs = 0.f;
+    int bi = INT_MAX;
+    for (int c = 0; c < n_chunks; ++c) state_merge(p[c].v, p[c].i, p[c].s, bv, bi, bs);
+    draft[e] = bi == INT_MAX ? 0 : bi;
+    conf[e] = bs > 0.f ? 1.0f / bs : 0.f;
+}
+
+static cudaLaunchConfig_t pdl_config(dim3 grid, dim3 block, size_t smem, cudaStream_t s, cudaLaunchAttribute* attr) {
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = s;
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cfg;
+}
+
 int32_t launch_accept(const __nv_bfloat16* logits, int64_t row_stride, int V, const int32_t* tokens,
                       const int32_t* parent, const int32_t* depth, const int32_t* tree_len, int B,
                       int gamma, int T_cap, int32_t* argmax_out, int32_t* accept_len, int32_t* path,
                       int32_t* bonus, int32_t* best_node, void* workspace, cudaStream_t s) {
     if (B == 0) return D2SD_OK;
-    const int n_chunks = ceil_div(V, kArgmaxChunk);
-    ArgPart* part = static_cast<ArgPart*>(workspace);
-    dim3 grid(B * T_cap, n_chunks);
-    argmax_partial_kernel<<<grid, kArgmaxThreads, 0, s>>>(logits, row_stride, V, tree_len, T_cap, n_chunks,
-                                                         part);
-    D2SD_CHECK_LAUNCH("argmax_partial_kernel");
-    accept_walk_kernel<<<B, 256, 3 * T_cap * sizeof(int32_t), s>>>(part, n_chunks, tokens, parent, depth,
-                                                                   tree_len, gamma, T_cap, argmax_out,
-                                                                   accept_len, path, bonus, best_node);
+    const int n_chunks = ceil_div(V, kScanChunk);
+    ScanPart* part = static_cast<ScanPart*>(workspace);
+    cudaLaunchAttribute attr[1];
+    cudaLaunchConfig_t cfg = pdl_config(dim3(B * T_cap, n_chunks), dim3(kScanThreads), 0, s, attr);
+    D2SD_CHECK_CUDA(cudaLaunchKernelEx(&cfg, vocab_scan_kernel<false>, logits, row_stride, V, tree_len, T_cap, n_chunks,
+                                       part));
+    D2SD_CHECK_LAUNCH("vocab_scan_kernel<argmax>");
+    cfg = pdl_config(dim3(B), dim3(256), 3 * T_cap * sizeof(int32_t), s, attr);
+    D2SD_CHECK_CUDA(cudaLaunchKernelEx(&cfg, accept_walk_kernel, (const ScanPart*)part, n_chunks, tokens, parent, depth,
+                                       tree_len, gamma, T_cap, argmax_out, accept_len, path, bonus, best_node));
     D2SD_CHECK_LAUNCH("accept_walk_kernel");
+    return D2SD_OK;
+}
+
+int32_t launch_confidence(const __nv_bfloat16* logits, int64_t row_stride, int V, const int32_t* anchor, int B,
+                          int gamma, int32_t* draft, float* conf, void* workspace, cudaStream_t s) {
+    if (B == 0) return D2SD_OK;
+    const int n_chunks = ceil_div(V, kScanChunk);
+    ScanPart* part = static_cast<ScanPart*>(workspace);
+    cudaLaunchAttribute attr[1];
+    cudaLaunchConfig_t cfg = pdl_config(dim3(B * (gamma - 1), n_chunks), dim3(kScanThreads), 0, s, attr);
+    D2SD_CHECK_CUDA(cudaLaunchKernelEx(&cfg, vocab_scan_kernel<true>, logits, row_stride, V, (const int32_t*)nullptr,
+                                       gamma - 1, n_chunks, part));
+    D2SD_CHECK_LAUNCH("vocab_scan_kernel<softmax>");
+    cfg = pdl_config(dim3(ceil_div(B * gamma, 128)), dim3(128), 0, s, attr);
+    D2SD_CHECK_CUDA(cudaLaunchKernelEx(&cfg, confidence_finish_kernel, (const ScanPart*)part, n_chunks, anchor, B, gamma,
+                                       draft, conf));
+    D2SD_CHECK_LAUNCH("confidence_finish_kernel");
     return D2SD_OK;
 }
 

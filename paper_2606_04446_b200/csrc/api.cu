@@ -276,7 +276,7 @@ int32_t d2sd_cascade_workspace_init(const d2sd_attn_params* p, void* workspace, 
 
 size_t d2sd_accept_workspace_bytes(int32_t B, int32_t T_cap, int32_t V) {
     if (B < 0 || T_cap < 1 || V < 1) return 0;
-    return align_up((size_t)B * T_cap * ceil_div(V, kArgmaxChunk) * 8, 256) + 256;
+    return align_up((size_t)B * T_cap * ceil_div(V, kScanChunk) * kScanPartBytes, 256) + 256;
 }
 
 int32_t d2sd_accept(const void* logits, int64_t row_stride, int32_t V, const int32_t* tokens,
@@ -290,7 +290,7 @@ int32_t d2sd_accept(const void* logits, int64_t row_stride, int32_t V, const int
     D2SD_CHECK_ARG(gamma >= 2 && gamma <= 64, "gamma = %d outside [2,64]", gamma);
     D2SD_CHECK_ARG(T_cap >= 1, "T_cap = %d", T_cap);
     D2SD_CHECK_SUPPORTED(T_cap <= 1024, "T_cap = %d > 1024", T_cap);
-    D2SD_CHECK_SUPPORTED(ceil_div(V, kArgmaxChunk) <= 65535, "V = %d too large", V);
+    D2SD_CHECK_SUPPORTED(ceil_div(V, kScanChunk) <= 65535, "V = %d too large", V);
     if (B == 0) return D2SD_OK;
     D2SD_CHECK_ARG(logits && tokens && parent && depth && tree_len && argmax_out && accept_len && path &&
                        bonus && best_node,
@@ -302,6 +302,118 @@ int32_t d2sd_accept(const void* logits, int64_t row_stride, int32_t V, const int
     return launch_accept(static_cast<const __nv_bfloat16*>(logits), row_stride, V, tokens, parent, depth,
                          tree_len, B, gamma, T_cap, argmax_out, accept_len, path, bonus, best_node, workspace,
                          static_cast<cudaStream_t>(stream));
+}
+
+size_t d2sd_confidence_workspace_bytes(int32_t B, int32_t gamma, int32_t V) {
+    if (B < 0 || gamma < 2 || V < 1) return 0;
+    return align_up((size_t)B * (gamma - 1) * ceil_div(V, kScanChunk) * kScanPartBytes, 256) + 256;
+}
+
+int32_t d2sd_draft_confidence(const void* logits, int64_t row_stride, int32_t V, const int32_t* anchor,
+                              int32_t B, int32_t gamma, int32_t* draft, float* conf, void* workspace,
+                              size_t workspace_bytes, void* stream) {
+    clear_error();
+    D2SD_CHECK_ARG(B >= 0 && V >= 1 && row_stride >= V, "B = %d, V = %d, row_stride = %lld", B, V,
+                   (long long)row_stride);
+    D2SD_CHECK_ARG(gamma >= 2 && gamma <= 64, "gamma = %d outside [2,64]", gamma);
+    D2SD_CHECK_SUPPORTED(ceil_div(V, kScanChunk) <= 65535, "V = %d too large", V);
+    if (B == 0) return D2SD_OK;
+    D2SD_CHECK_ARG(logits && anchor && draft && conf, "a required buffer is NULL");
+    if (workspace == nullptr || workspace_bytes < d2sd_confidence_workspace_bytes(B, gamma, V) ||
+        (reinterpret_cast<uintptr_t>(workspace) & 15))
+        return set_error(D2SD_ERR_WORKSPACE, "confidence workspace %p with %zu bytes; need %zu, 16-byte aligned",
+                         workspace, workspace_bytes, d2sd_confidence_workspace_bytes(B, gamma, V));
+    return launch_confidence(static_cast<const __nv_bfloat16*>(logits), row_stride, V, anchor, B, gamma, draft, conf,
+                             workspace, static_cast<cudaStream_t>(stream));
+}
+
+size_t d2sd_commit_workspace_bytes(int32_t B) {
+    if (B < 0) return 0;
+    return align_up((size_t)(B + 1) * sizeof(int32_t), 256);
+}
+
+int32_t d2sd_commit_kv(const d2sd_commit_params* p, const void* tree_k, const void* tree_v, const int32_t* path,
+                       const int32_t* accept_len, const int32_t* ctx_len, void* k_cache, void* v_cache,
+                       const int32_t* kv_indptr, int32_t* kv_indices, const int32_t* free_pages, int32_t n_free,
+                       int32_t* free_head, int32_t* ctx_len_out, int32_t* dropped, const void* feat, void* feat_out,
+                       void* workspace, size_t workspace_bytes, void* stream) {
+    clear_error();
+    D2SD_CHECK_ARG(p != nullptr, "params is NULL");
+    D2SD_CHECK_ARG(p->B >= 0 && p->T_cap >= 1 && p->Hkv >= 1 && p->d >= 1 && p->n_layers >= 0,
+                   "B = %d, T_cap = %d, Hkv = %d, d = %d, n_layers = %d", p->B, p->T_cap, p->Hkv, p->d, p->n_layers);
+    D2SD_CHECK_ARG(p->gamma >= 2 && p->gamma <= 64, "gamma = %d outside [2,64]", p->gamma);
+    D2SD_CHECK_ARG(p->page_size >= 0 && p->kv_rows >= 0 && p->F >= 0, "page_size = %d, kv_rows = %lld, F = %d",
+                   p->page_size, (long long)p->kv_rows, p->F);
+    D2SD_CHECK_SUPPORTED(p->B <= 65535 && p->n_layers <= 65535, "B = %d / n_layers = %d > 65535", p->B, p->n_layers);
+    const int64_t row_elems = (int64_t)p->Hkv * p->d;
+    D2SD_CHECK_SUPPORTED(row_elems % 8 == 0 && p->F % 8 == 0, "Hkv*d = %lld and F = %d must be multiples of 8",
+                         (long long)row_elems, p->F);
+    D2SD_CHECK_ARG(p->tree_layer_stride >= (int64_t)p->B * p->T_cap * row_elems && p->tree_layer_stride % 8 == 0,
+                   "tree_layer_stride = %lld", (long long)p->tree_layer_stride);
+    D2SD_CHECK_ARG(p->cache_layer_stride >= p->kv_rows * row_elems && p->cache_layer_stride % 8 == 0,
+                   "cache_layer_stride = %lld", (long long)p->cache_layer_stride);
+    if (p->B == 0 || p->n_layers == 0) return D2SD_OK;
+    D2SD_CHECK_ARG(tree_k && tree_v && path && accept_len && ctx_len && k_cache && v_cache && ctx_len_out && dropped,
+                   "a required buffer is NULL");
+    D2SD_CHECK_ARG(kv_indptr != nullptr || (p->B == 1 && p->page_size == 0),
+                   "kv_indptr may be NULL only for B == 1 contiguous KV");
+    D2SD_CHECK_ARG((p->page_size > 0) == (kv_indices != nullptr), "kv_indices must be given exactly when page_size > 0");
+    D2SD_CHECK_ARG((free_pages != nullptr) == (free_head != nullptr) && n_free >= 0 && (free_pages || n_free == 0),
+                   "free_pages / free_head must be given together (n_free = %d)", n_free);
+    D2SD_CHECK_ARG(free_pages == nullptr || p->page_size > 0, "a free list needs paged KV");
+    D2SD_CHECK_ARG((feat != nullptr) == (feat_out != nullptr) && ((feat != nullptr) == (p->F > 0)),
+                   "feat / feat_out / F must be given together");
+    const uintptr_t al = reinterpret_cast<uintptr_t>(tree_k) | reinterpret_cast<uintptr_t>(tree_v) |
+                         reinterpret_cast<uintptr_t>(k_cache) | reinterpret_cast<uintptr_t>(v_cache) |
+                         reinterpret_cast<uintptr_t>(feat) | reinterpret_cast<uintptr_t>(feat_out);
+    D2SD_CHECK_ARG((al & 15) == 0, "tree_k/tree_v/k_cache/v_cache/feat/feat_out must be 16-byte aligned");
+    if (workspace == nullptr || workspace_bytes < d2sd_commit_workspace_bytes(p->B) ||
+        (reinterpret_cast<uintptr_t>(workspace) & 15))
+        return set_error(D2SD_ERR_WORKSPACE, "commit workspace %p with %zu bytes; need %zu, 16-byte aligned", workspace,
+                         workspace_bytes, d2sd_commit_workspace_bytes(p->B));
+    CommitArgs a{};
+    a.tree_k = static_cast<const __nv_bfloat16*>(tree_k);
+    a.tree_v = static_cast<const __nv_bfloat16*>(tree_v);
+    a.tree_layer_stride = p->tree_layer_stride;
+    a.path = path; a.accept_len = accept_len; a.ctx_len = ctx_len;
+    a.k_cache = static_cast<__nv_bfloat16*>(k_cache);
+    a.v_cache = static_cast<__nv_bfloat16*>(v_cache);
+    a.cache_layer_stride = p->cache_layer_stride; a.kv_rows = p->kv_rows;
+    a.kv_indptr = kv_indptr; a.kv_indices = kv_indices; a.page_size = p->page_size;
+    a.free_pages = free_pages; a.n_free = n_free; a.free_head = free_head;
+    a.B = p->B; a.gamma = p->gamma; a.T_cap = p->T_cap; a.Hkv = p->Hkv; a.d = p->d; a.n_layers = p->n_layers;
+    a.ctx_len_out = ctx_len_out; a.dropped = dropped;
+    a.feat = static_cast<const __nv_bfloat16*>(feat);
+    a.feat_out = static_cast<__nv_bfloat16*>(feat_out);
+    a.F = p->F;
+    a.n_fit = static_cast<int32_t*>(workspace);
+    return launch_commit_kv(a, static_cast<cudaStream_t>(stream));
+}
+
+int32_t d2sd_select_third(const float* conf2, const int32_t* prefix_len, int32_t B, int32_t gamma, int32_t K,
+                          int32_t* third_len, double* r3_out, void* stream) {
+    clear_error();
+    if (int32_t st = check_block(B, gamma, K)) return st;
+    if (B == 0 || K == 0) return D2SD_OK;
+    D2SD_CHECK_ARG(conf2 && prefix_len && third_len, "a required buffer is NULL");
+    return launch_select_third(conf2, prefix_len, B, gamma, K, third_len, r3_out, static_cast<cudaStream_t>(stream));
+}
+
+int32_t d2sd_build_tree3(const int32_t* draft1, const int32_t* draft2, const int32_t* draft3,
+                         const int32_t* prefix_len, const int32_t* third_len, const int32_t* ctx_len, int32_t B,
+                         int32_t gamma, int32_t K, int32_t T_cap, int32_t* tokens, int32_t* parent, int32_t* depth,
+                         int32_t* pos_id, int32_t* branch_off, uint32_t* mask, int32_t* tree_len, void* stream) {
+    clear_error();
+    if (int32_t st = check_block(B, gamma, K)) return st;
+    const int need = gamma + K * (gamma - 1) - K * (K - 1) / 2 + K * (gamma - 2) - K * (K - 1) / 2;
+    D2SD_CHECK_ARG(T_cap >= need, "T_cap = %d < largest depth-3 tree %d for gamma = %d, K = %d", T_cap, need, gamma, K);
+    D2SD_CHECK_SUPPORTED(T_cap <= 1024, "T_cap = %d > 1024", T_cap);
+    if (B == 0) return D2SD_OK;
+    D2SD_CHECK_ARG(draft1 && ctx_len && tokens && parent && depth && pos_id && branch_off && mask && tree_len,
+                   "a required buffer is NULL");
+    D2SD_CHECK_ARG(K == 0 || (draft2 && draft3 && prefix_len && third_len), "draft2 / draft3 / prefix_len / third_len is NULL with K = %d", K);
+    return launch_build_tree3(draft1, draft2, draft3, prefix_len, third_len, ctx_len, B, gamma, K, T_cap, tokens, parent,
+                              depth, pos_id, branch_off, mask, tree_len, static_cast<cudaStream_t>(stream));
 }
 
 }  // extern "C"

@@ -67,11 +67,40 @@ int32_t launch_build_tree(const int32_t* draft1, const int32_t* draft2, const in
                           int32_t* parent, int32_t* depth, int32_t* pos_id, int32_t* branch_off,
                           uint32_t* mask, int32_t* tree_len, cudaStream_t s);
 
-constexpr int kArgmaxChunk = 8192;  // vocabulary elements scanned per CTA
+constexpr int kScanChunk = 16384;  // vocabulary elements scanned per CTA (accept.cu)
+constexpr size_t kScanPartBytes = 16;
 int32_t launch_accept(const __nv_bfloat16* logits, int64_t row_stride, int V, const int32_t* tokens,
                       const int32_t* parent, const int32_t* depth, const int32_t* tree_len, int B,
                       int gamma, int T_cap, int32_t* argmax_out, int32_t* accept_len, int32_t* path,
                       int32_t* bonus, int32_t* best_node, void* workspace, cudaStream_t s);
+int32_t launch_confidence(const __nv_bfloat16* logits, int64_t row_stride, int V, const int32_t* anchor, int B,
+                          int gamma, int32_t* draft, float* conf, void* workspace, cudaStream_t s);
+int32_t launch_select_third(const float* conf2, const int32_t* prefix_len, int B, int gamma, int K,
+                            int32_t* third_len, double* r3_out, cudaStream_t s);
+int32_t launch_build_tree3(const int32_t* draft1, const int32_t* draft2, const int32_t* draft3,
+                           const int32_t* prefix_len, const int32_t* third_len, const int32_t* ctx_len, int B,
+                           int gamma, int K, int T_cap, int32_t* tokens, int32_t* parent, int32_t* depth,
+                           int32_t* pos_id, int32_t* branch_off, uint32_t* mask, int32_t* tree_len, cudaStream_t s);
+struct CommitArgs {
+    const __nv_bfloat16 *tree_k, *tree_v;
+    int64_t tree_layer_stride;  // elements
+    const int32_t *path, *accept_len, *ctx_len;
+    __nv_bfloat16 *k_cache, *v_cache;
+    int64_t cache_layer_stride, kv_rows;
+    const int32_t* kv_indptr;
+    int32_t* kv_indices;
+    int page_size;
+    const int32_t* free_pages;
+    int n_free;
+    int32_t* free_head;
+    int B, gamma, T_cap, Hkv, d, n_layers;
+    int32_t *ctx_len_out, *dropped;
+    const __nv_bfloat16* feat;  // optional [B,T_cap,F]
+    __nv_bfloat16* feat_out;    // optional [B,gamma,F]
+    int F;
+    int32_t* n_fit;             // workspace [B]
+};
+int32_t launch_commit_kv(const CommitArgs& a, cudaStream_t s);
 
 // Partial softmax states in the workspace.
 //  mma.sync path ("row layout"): O fp32 [B][NS][T_cap][Hq][d], LSE fp32 [B][NS][T_cap][Hq]; slots
