@@ -258,7 +258,7 @@ class Workload:
 
     @property
     def attn_kernel(self) -> str:
-        return "attn_cascade_tc_kernel"
+        return "attn_stream_kernel"
 
     @property
     def launches_per_step(self) -> int:

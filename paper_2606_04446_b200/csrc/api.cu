@@ -47,7 +47,7 @@ static int32_t make_plan(const d2sd_attn_params* p, AttnPlan* out) {
                    p->Hq, p->Hkv);
     D2SD_CHECK_ARG(p->max_ctx_len >= 0 && p->kv_rows >= 0, "max_ctx_len = %d, kv_rows = %lld",
                    p->max_ctx_len, (long long)p->kv_rows);
-    D2SD_CHECK_ARG(p->num_splits >= 0 && p->impl >= 0 && p->impl <= 2, "num_splits = %d, impl = %d",
+    D2SD_CHECK_ARG(p->num_splits >= 0 && p->impl >= 0 && p->impl <= 3, "num_splits = %d, impl = %d",
                    p->num_splits, p->impl);
     D2SD_CHECK_ARG(p->phases >= 0 && p->phases <= 7, "phases = %d outside [0,7]", p->phases);
     D2SD_CHECK_SUPPORTED(p->d == 128, "head dim %d: only 128 is built", p->d);
@@ -63,14 +63,85 @@ static int32_t make_plan(const d2sd_attn_params* p, AttnPlan* out) {
     pl.max_ctx_len = p->max_ctx_len;
     pl.kv_rows = p->kv_rows;
     pl.use_tc = false;
-    if (p->impl != 1) {
+    pl.use_stream = false;
+    if (p->impl == 3 || p->impl == 0) {
+        pl.use_stream = attn_stream_supported(pl);
+        D2SD_CHECK_SUPPORTED(pl.use_stream || p->impl != 3, "impl = 3 (one-tile-per-CTA tcgen05 kernel) does not cover this shape");
+    } else if (p->impl != 1) {
         pl.use_tc = attn_cascade_tc_supported(pl);
         D2SD_CHECK_SUPPORTED(pl.use_tc || p->impl != 2, "impl = 2 (tcgen05) does not cover this shape");
     }
     const int rows = pl.T_cap * pl.G;
     const int max_ctx = p->max_ctx_len > 0 ? p->max_ctx_len : 1;
     int splits = p->num_splits;
-    if (pl.use_tc) {
+    if (pl.use_stream) {
+        // One CTA = (request, kv head, M tile, context chunk).  M tiles (2p, 2p+1) over the same chunk form a
+        // 2-CTA cluster that shares its key tiles; an odd last tile's chunks are paired without sharing.
+        // One wave (enough SMs for every M tile of every (request, kv head)): the chunk counts are chosen
+        // from a cost model (cycles per unit, fixed cost of the partial-state exchange) so that paired tiles
+        // and the usually short last tile finish together; every request cuts its own key tiles evenly
+        // (tps_min = 1).  Otherwise: fixed chunks of 32 key tiles, several waves.
+        const int n_mt = ceil_div(rows, 128);
+        const int n_pairs = n_mt / 2, odd = n_mt & 1;
+        const int max_tiles = ceil_div(p->max_ctx_len, 128) + ceil_div(pl.T_cap, 128);
+        const int64_t heads = (int64_t)pl.B * pl.Hkv;
+        const int budget = (int)((sm_count() & ~1) / (heads > 0 ? heads : 1));
+        int ca = 1, cb = 1;
+        pl.tps_min = 1;
+        if (splits > 0) {
+            ca = cb = splits;
+        } else if (budget >= 2 * n_pairs + 2 * odd) {
+            const int rows_last = rows - (n_mt - 1) * 128;
+            const double ua = 1250.0, ub = (odd && rows_last <= 32) ? 1050.0 : 1250.0;
+            const double xa = 3000.0, xb = 500.0 + 3000.0 * (odd ? rows_last : 128) / 128.0;
+            auto cost = [&](int c, double u, double x) { return ceil_div(max_tiles, c) * u + (c > 1 ? x : 0.0); };
+            double best = 1e30;
+            const int ca_max = n_pairs ? (budget - 2 * odd) / (2 * n_pairs) : 1;
+            for (int a2 = 1; a2 <= (n_pairs ? ca_max : 1) && a2 <= 64; ++a2) {
+                int b_room = odd ? ((budget - 2 * n_pairs * a2) & ~1) : 0;
+                if (b_room > 64) b_room = 64;
+                double tb = 0.0;
+                int b_best = 1;
+                if (odd) {
+                    tb = 1e30;
+                    for (int b2 = 1; b2 <= b_room; ++b2) {
+                        const double t = cost(b2, ub, xb);
+                        if (t < tb) { tb = t; b_best = b2; }
+                    }
+                }
+                const double ta = n_pairs ? cost(a2, ua, xa) : 0.0;
+                const double t = ta > tb ? ta : tb;
+                if (t < best) { best = t; ca = a2; cb = b_best; }
+            }
+        } else {
+            ca = cb = ceil_div(max_tiles, 32);
+            pl.tps_min = -1;  // fixed below
+        }
+        if (ca > 64) ca = 64;  // a group's CTAs wait for each other
+        if (cb > 64) cb = 64;
+        if (ca > max_tiles) ca = max_tiles;  // never an always-empty chunk
+        if (cb > max_tiles) cb = max_tiles;
+        if (ca < 1) ca = 1;
+        if (cb < 1) cb = 1;
+        if (pl.tps_min < 0) pl.tps_min = ceil_div(max_tiles, ca);
+        pl.n_mt = n_mt;
+        pl.n_pair = n_pairs; pl.n_single = odd;
+        pl.chunks_a = ca;
+        pl.chunks_b = cb;
+        pl.chunk_keys = 0;
+        pl.num_splits = n_pairs ? ca : cb;
+        pl.NS = 0;
+        pl.grp_rows = 128 * (ca > cb ? ca : cb);
+        const size_t n_groups = (size_t)pl.B * pl.Hkv * n_mt;
+        const size_t slot_rows = n_groups * pl.grp_rows;
+        D2SD_CHECK_SUPPORTED(n_groups * 2 * sizeof(unsigned) <= kWsHeaderBytes - 16, "B*Hkv*tiles = %zu groups > %zu",
+                             n_groups, (kWsHeaderBytes - 16) / (2 * sizeof(unsigned)));
+        pl.off_cnt = 0;
+        pl.cnt_bytes = kWsHeaderBytes;
+        pl.off_o = pl.cnt_bytes;
+        pl.off_lse = pl.off_o + align_up(slot_rows * pl.d * sizeof(float), 256);
+        pl.bytes = pl.off_lse + align_up(slot_rows * sizeof(float), 256);
+    } else if (pl.use_tc) {
         // Query tiles (2p, 2p+1) form pair items, an odd last tile the single item; every item gets its
         // own run of context chunks (one CTA each).  A pair item does two units per key tile, a single
         // item one, so the single item gets about half as many chunks.  With enough SMs for one wave the
@@ -241,6 +312,17 @@ int32_t d2sd_cascade_verify_attn(const d2sd_attn_params* p, const void* q, const
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     const int phases = p->phases ? p->phases : 7;
     const bool do_prefix = phases & 1, do_tree = phases & 2, do_merge = phases & 4;
+    if (pl.use_stream) {
+        a.counters = reinterpret_cast<unsigned*>(static_cast<char*>(workspace) + pl.off_cnt);
+        if (dbg_state) {
+            const size_t half = (size_t)pl.B * pl.T_cap * pl.Hq * (pl.d + 1);
+            if (int32_t st = launch_attn_stream(pl, a, 1, dbg_state, s)) return st;
+            if (int32_t st = launch_attn_stream(pl, a, 2, dbg_state + half, s)) return st;
+        }
+        const int mode = phases & 3;
+        if (mode == 0) return D2SD_OK;
+        return launch_attn_stream(pl, a, mode, nullptr, s);
+    }
     if (pl.use_tc) {
         // One fused launch: prefix tiles, tree tiles and the cascade merge.  phases selects which key
         // tiles take part (1 = prefix only, 2 = tree only); dbg_state costs two extra launches.

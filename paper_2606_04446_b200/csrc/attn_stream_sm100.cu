@@ -1,0 +1,1066 @@
+// Stage (c), fused: cascade tree-verify attention in ONE launch on tcgen05 / TMEM / TMA (sm_100a).
+// PAPER.md:52, :124, :154.
+//
+// Every tree query of every branch and every GQA head of one kv head is a row of one batched query
+// matrix (row r = t*G + hh), cut into 128-row M tiles.  The keys of a request are the committed
+// prefix followed by the tree-local keys, cut into 128-key tiles: prefix tiles 0..np-1
+// (np = ceil(L/128)) and tree tiles np..np+nt-1 (nt = ceil(T/128)); a tree tile is an ordinary key
+// tile whose scores additionally pass the node's ancestor-mask bits.
+//
+// Work decomposition.  One CTA serves (request b, kv head g, M tile, context chunk): ONE query tile and
+// a run of key tiles ("units").  The launch is made of 2-CTA clusters: the CTAs of M tiles (2p, 2p+1)
+// over the same chunk form a SHARING pair -- rank 0 loads every K tile, rank 1 every V tile, each TMA
+// multicast into both CTAs' rings, so a KV tile crosses the L2->SM fabric once per 256 query rows --
+// and the chunks of an odd last M tile are paired without sharing.
+//
+// TMEM (512 columns): O (128 fp32 columns), S_0, S_1 (128 each), P_0, P_1 (64 each, bf16 pairs).
+// Unit n uses buffers n & 1.  S and P are separate columns, so Q.K^T of unit n+2 is issued as soon as
+// the softmax has READ S_n (it does not wait for P.V of unit n), and the softmax never waits for the
+// tensor pipe in steady state:
+//
+//   S_n[128 x 128] = Q[128 x 128] . K_n^T        tcgen05.mma, A/B from 128B-swizzled SMEM (TMA)
+//   P_n            = exp2(c*(S_n - m_ref))       one softmax thread per row (TMEM lane)
+//   O[128 x 128]  += P_n[128 x 128] . V_n        tcgen05.mma, A = P from TMEM, B = V (MN-major SMEM)
+//
+// Warp roles (384 threads): warps 0..3 = softmax team A (even units), warps 4..7 = team B (odd units),
+// thread (w, lane) of either team owns query row w*32 + lane; warp 8 = K producer (+ Q), warp 9 =
+// V producer (also zeroes the V rows behind a ragged tile end: they are multiplied by exact zeros
+// and may hold anything, NaN included), warp 10 = MMA issuer (one elected thread; owns the TMEM
+// allocation), warp 11 idle.  The two teams work on different units at the same time, so one team's
+// loads / maxima / packs overlap the other's exponentials on the shared MUFU pipe.
+//
+// One accumulator, two teams: the row's reference maximum m_ref travels with the unit sequence.  The
+// owner of unit n reads m_ref(n-1) from shared memory (published by the other team, ordered by a
+// 64-thread named barrier per warp pair), raises it only when the tile maximum exceeds it by more than
+// 2^8 (lazy rescale), publishes m_ref(n), and -- only when it raised it -- waits for P.V of unit n-1
+// and rescales its O row in TMEM before it releases P_n.  Each thread keeps its own row sum relative
+// to the last reference it has seen; the two sums meet in the epilogue.
+//
+// Cascade merge in the same launch (log-sum-exp state merge): every CTA writes its
+// normalised partial state (O fp32, LSE) to the workspace straight from registers (tcgen05.ld 16x256b
+// gives four adjacent lanes 32 contiguous bytes of a row: full-sector stores; it stays in L2),
+// publishes it with a release-increment of its group's arrival counter (group = request, kv head,
+// M tile), waits until all non-empty chunks of the group have arrived, and merges ITS share of the
+// group's rows (coalesced 16-byte loads, all in flight at once).  The counters reset themselves.
+// The wait needs the group's CTAs (<= 64) to be co-resident; the plan sizes one-wave grids so that
+// they are, multi-wave grids are safe because a group is a run of consecutive blocks of the grid's
+// linear order.  A wait that does not end sets an error word in the workspace header instead of
+// trapping (d2sd.h).
+// The launch is a programmatic dependent launch: the prologue (barriers, TMEM, tensor-map prefetch)
+// overlaps the tail of the preceding kernel; no global memory is touched before griddepcontrol.wait.
+#include <cuda.h>
+
+#include "common.cuh"
+
+namespace d2sd {
+namespace {
+
+constexpr int kD = 128;
+constexpr int kTileM = 128;
+constexpr int kTileN = 128;
+constexpr int kRingK = 3, kRingV = 3;  // K tiles / V tiles in flight or in use
+constexpr int kThreads = 384;
+constexpr uint32_t kQTileBytes = kTileM * kD * 2;   // 32 KiB: [d_hi 2][128 rows][128 B]
+constexpr uint32_t kKvTileBytes = kTileN * kD * 2;  // 32 KiB: [d_hi 2][128 keys][128 B]
+constexpr uint32_t kOffQ = 0;
+constexpr uint32_t kOffK = kQTileBytes;
+constexpr uint32_t kOffV = kOffK + kRingK * kKvTileBytes;
+constexpr uint32_t kOffBar = kOffV + kRingV * kKvTileBytes;
+constexpr uint32_t kOffX = kOffBar + 256;                 // reference-maximum hand-off: fp32 [2 teams][128 rows]
+constexpr uint32_t kOffXL = kOffX + 2 * kTileM * 4;         // row sums of the two teams: fp32 [2][128]
+constexpr uint32_t kSmemUsed = kOffXL + 2 * kTileM * 4;
+constexpr uint32_t kSmemBytes = 232448;                   // the whole 227 KiB: kSmemUsed + alignment slack
+constexpr uint32_t kTmemCols = 512;
+constexpr uint32_t kTmemS = 128;   // S_0, S_1 behind O
+constexpr uint32_t kTmemP = 384;   // P_0, P_1 (64 columns each)
+constexpr float kLog2e = 1.4426950408889634f;
+constexpr float kRescaleThreshold = 8.0f;  // log2 units
+constexpr uint32_t kRegsControl = 80, kRegsSoftmax = 208;  // setmaxnreg targets
+
+// barrier slots (8 bytes each) at kOffBar
+enum : uint32_t {
+    kBarQFull = 0,
+    kBarKFull = 1,                       // [kRingK]
+    kBarKEmpty = kBarKFull + kRingK,     // [kRingK]
+    kBarVFull = kBarKEmpty + kRingK,     // [kRingV]
+    kBarVEmpty = kBarVFull + kRingV,     // [kRingV]
+    kBarSFull = kBarVEmpty + kRingV,     // [2] Q.K^T of a unit has completed
+    kBarSFree = kBarSFull + 2,           // [2] the owning team has read S into registers
+    kBarPFull = kBarSFree + 2,           // [2][4] P is released to the tensor pipe in four 32-key pieces
+    kBarPFree = kBarPFull + 8,           // [2] P.V of a unit has completed (P buffer reusable, O current)
+    kBarVFix = kBarPFree + 2,            // [2] V rows behind a ragged tile end are zero (<= 2 ragged tiles per CTA)
+    kBarAllDone = kBarVFix + 2,
+    kNumBars = kBarAllDone + 1,
+    kTmemSlot = kNumBars  // uint32 written by tcgen05.alloc
+};
+static_assert((kNumBars + 1) * 8 <= 256, "barrier area");
+static_assert(kSmemUsed + 768 <= kSmemBytes, "shared memory budget");  // the kernel checks the actual alignment slack
+
+// ---- PTX wrappers -------------------------------------------------------------------------------
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
+// Bounded wait: a protocol bug traps (reported as a launch failure) instead of hanging the GPU.
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    uint32_t spins = 0;
+    while (!mbar_try_wait(bar, parity)) {
+        if (++spins > (1u << 26)) __trap();
+    }
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_commit(uint32_t bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap* tm, uint32_t bar, int c0, int c1, int c2,
+                                            int c3, uint64_t hint) {
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint"
+        " [%0], [%1, {%3, %4, %5, %6}], [%2], %7;" ::"r"(dst),
+        "l"(reinterpret_cast<uint64_t>(tm)), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "l"(hint)
+        : "memory");
+}
+__device__ __forceinline__ void tma_load_5d(uint32_t dst, const CUtensorMap* tm, uint32_t bar, int c0, int c1, int c2,
+                                            int c3, int c4, uint64_t hint) {
+    asm volatile(
+        "cp.async.bulk.tensor.5d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint"
+        " [%0], [%1, {%3, %4, %5, %6, %7}], [%2], %8;" ::"r"(dst),
+        "l"(reinterpret_cast<uint64_t>(tm)), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4), "l"(hint)
+        : "memory");
+}
+__device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* tm) {
+    asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(tm)) : "memory");
+}
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void named_bar_arrive(uint32_t id, uint32_t threads) {
+    asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(threads) : "memory");
+}
+__device__ __forceinline__ void named_bar_sync(uint32_t id, uint32_t threads) {
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
+}
+constexpr uint64_t kEvictNormal = 0x1000000000000000ull;  // KV: read by the 2-3 sibling CTAs of the kv head within a few
+                                                          // microseconds (evict-first measured 3% slower on configs 3, 4)
+constexpr uint64_t kEvictLast = 0x14F0000000000000ull;   // re-read by every chunk CTA of the head: Q
+
+// D[tmem] (+)= A[smem] . B[smem]
+__device__ __forceinline__ void umma_ss(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc,
+                                        uint32_t accumulate) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem),
+        "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+// D[tmem] (+)= A[tmem] . B[smem]
+__device__ __forceinline__ void umma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc,
+                                        uint32_t accumulate) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}" ::"r"(d_tmem),
+        "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+
+// Shared-memory matrix descriptor, 128B swizzle, descriptor version 1 (Blackwell).
+//   K-major  operand: rows of 128 B (64 bf16 along K); 8-row groups SBO = 1024 B apart; LBO unused (1).
+//   MN-major operand: rows of 128 B (64 bf16 along MN); the next 64 along MN is LBO bytes away, the next
+//                     8 along K is SBO = 1024 B away.
+// The start-address field holds (addr >> 4); advancing an operand by `bytes` adds (bytes >> 4).
+__device__ __forceinline__ uint64_t smem_desc(uint32_t addr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
+    return (uint64_t)((addr & 0x3FFFFu) >> 4) | ((uint64_t)(lbo_bytes >> 4) << 16) |
+           ((uint64_t)(sbo_bytes >> 4) << 32) | (1ull << 46) | (2ull << 61);
+}
+// Instruction descriptor, kind::f16: fp32 accumulate, bf16 x bf16.
+__host__ __device__ constexpr uint32_t idesc(uint32_t M, uint32_t N, uint32_t b_mn_major) {
+    return (1u << 4) | (1u << 7) | (1u << 10) | (b_mn_major << 16) | ((N >> 3) << 17) | ((M >> 4) << 24);
+}
+constexpr uint32_t kIdescPV = idesc(kTileM, kD, 1);
+
+#define D2SD_R32(r, o)                                                                                     \
+    "=r"(r[o + 0]), "=r"(r[o + 1]), "=r"(r[o + 2]), "=r"(r[o + 3]), "=r"(r[o + 4]), "=r"(r[o + 5]),         \
+        "=r"(r[o + 6]), "=r"(r[o + 7]), "=r"(r[o + 8]), "=r"(r[o + 9]), "=r"(r[o + 10]), "=r"(r[o + 11]),   \
+        "=r"(r[o + 12]), "=r"(r[o + 13]), "=r"(r[o + 14]), "=r"(r[o + 15]), "=r"(r[o + 16]), "=r"(r[o + 17]), \
+        "=r"(r[o + 18]), "=r"(r[o + 19]), "=r"(r[o + 20]), "=r"(r[o + 21]), "=r"(r[o + 22]), "=r"(r[o + 23]), \
+        "=r"(r[o + 24]), "=r"(r[o + 25]), "=r"(r[o + 26]), "=r"(r[o + 27]), "=r"(r[o + 28]), "=r"(r[o + 29]), \
+        "=r"(r[o + 30]), "=r"(r[o + 31])
+#define D2SD_W32(r, o)                                                                                     \
+    "r"(r[o + 0]), "r"(r[o + 1]), "r"(r[o + 2]), "r"(r[o + 3]), "r"(r[o + 4]), "r"(r[o + 5]), "r"(r[o + 6]),   \
+        "r"(r[o + 7]), "r"(r[o + 8]), "r"(r[o + 9]), "r"(r[o + 10]), "r"(r[o + 11]), "r"(r[o + 12]),         \
+        "r"(r[o + 13]), "r"(r[o + 14]), "r"(r[o + 15]), "r"(r[o + 16]), "r"(r[o + 17]), "r"(r[o + 18]),      \
+        "r"(r[o + 19]), "r"(r[o + 20]), "r"(r[o + 21]), "r"(r[o + 22]), "r"(r[o + 23]), "r"(r[o + 24]),      \
+        "r"(r[o + 25]), "r"(r[o + 26]), "r"(r[o + 27]), "r"(r[o + 28]), "r"(r[o + 29]), "r"(r[o + 30]),      \
+        "r"(r[o + 31])
+#define D2SD_TMEM_LD32(taddr, r, o)                                                                         \
+    asm volatile(                                                                                           \
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,"    \
+        "%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"                          \
+        : D2SD_R32(r, o)                                                                                    \
+        : "r"(taddr))
+#define D2SD_TMEM_ST32(taddr, r, o)                                                                         \
+    asm volatile(                                                                                           \
+        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15," \
+        "%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31,%32};" ::"r"(taddr),               \
+        D2SD_W32(r, o)                                                                                      \
+        : "memory")
+#define D2SD_TMEM_ST16(taddr, r)                                                                            \
+    asm volatile(                                                                                           \
+        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15," \
+        "%16};" ::"r"(taddr),                                                                               \
+        "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]),   \
+        "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])                    \
+        : "memory")
+// Scheduling fence for 32 registers: the values are "rewritten" here, \
+        so everything computed from them
+// stays behind the preceding asm volatile statements (the compiler would otherwise hoist all 128
+// exponentials above the first piece-wise release of P).
+#define D2SD_PIN32(r, \
+        o) asm volatile("" : \
+        "+r"(r[o + 0]), \
+        "+r"(r[o + 1]), \
+        "+r"(r[o + 2]), \
+        "+r"(r[o + 3]), \
+        "+r"(r[o + 4]), \
+        "+r"(r[o + 5]), \
+        "+r"(r[o + 6]), \
+        "+r"(r[o + 7]), \
+        "+r"(r[o + 8]), \
+        "+r"(r[o + 9]), \
+        "+r"(r[o + 10]), \
+        "+r"(r[o + 11]), \
+        "+r"(r[o + 12]), \
+        "+r"(r[o + 13]), \
+        "+r"(r[o + 14]), \
+        "+r"(r[o + 15]), \
+        "+r"(r[o + 16]), \
+        "+r"(r[o + 17]), \
+        "+r"(r[o + 18]), \
+        "+r"(r[o + 19]), \
+        "+r"(r[o + 20]), \
+        "+r"(r[o + 21]), \
+        "+r"(r[o + 22]), \
+        "+r"(r[o + 23]), \
+        "+r"(r[o + 24]), \
+        "+r"(r[o + 25]), \
+        "+r"(r[o + 26]), \
+        "+r"(r[o + 27]), \
+        "+r"(r[o + 28]), \
+        "+r"(r[o + 29]), \
+        "+r"(r[o + 30]), \
+        "+r"(r[o + 31]))
+__device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+
+__device__ __forceinline__ float ex2(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+// Same, but ordered against the other volatile statements (TMEM stores / waits, barrier arrivals): the
+// softmax loop uses it to keep a piece's exponentials ahead of the wait for the previous piece's store.
+__device__ __forceinline__ float ex2_ordered(float x) {
+    float y;
+    asm volatile("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ uint32_t pack2_bf16(float lo, float hi) {
+    __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
+    return *reinterpret_cast<uint32_t*>(&v);
+}
+
+// One lane of a fully active warp; unlike `lane == 0` it lets ptxas keep the MMA operands on the uniform
+// datapath (no per-instruction elect loop around every tcgen05.mma).
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+    return pred != 0;
+}
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+// shared -> global bulk copy (bytes % 16 == 0), one bulk group per call site
+__device__ __forceinline__ void bulk_store(void* gdst, uint32_t ssrc, uint32_t bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(ssrc), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+
+
+
+// ---- cluster (2-CTA sharing pair) ---------------------------------------------------------------
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ void cluster_sync_all() {  // every thread of both CTAs
+    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// tcgen05.commit that arrives on the barrier at the same offset in every CTA of `mask`
+__device__ __forceinline__ void tc_commit_mc(uint32_t bar, uint16_t mask) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(bar),
+                 "h"(mask)
+                 : "memory");
+}
+__device__ __forceinline__ void tma_load_4d_mc(uint32_t dst, const CUtensorMap* tm, uint32_t bar, int c0, int c1, int c2,
+                                               int c3, uint16_t mask, uint64_t hint) {
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster.L2::cache_hint"
+        " [%0], [%1, {%3, %4, %5, %6}], [%2], %7, %8;" ::"r"(dst),
+        "l"(reinterpret_cast<uint64_t>(tm)), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "h"(mask), "l"(hint)
+        : "memory");
+}
+__device__ __forceinline__ void tma_load_5d_mc(uint32_t dst, const CUtensorMap* tm, uint32_t bar, int c0, int c1, int c2,
+                                               int c3, int c4, uint16_t mask, uint64_t hint) {
+    asm volatile(
+        "cp.async.bulk.tensor.5d.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster.L2::cache_hint"
+        " [%0], [%1, {%3, %4, %5, %6, %7}], [%2], %8, %9;" ::"r"(dst),
+        "l"(reinterpret_cast<uint64_t>(tm)), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4), "h"(mask), "l"(hint)
+        : "memory");
+}
+
+// What one CTA does: which M tile / chunk, which key tiles it streams, whom it shares them with.
+struct Work {
+    int b, g, tile, chunk;
+    int share;         // 1: sharing pair (this CTA and its cluster peer stream the same key tiles)
+    int rank;          // rank in the cluster (sharing pair: 0 loads K, 1 loads V)
+    int row_base;      // first query row (t*G + hh) of the tile
+    int rows;          // valid query rows of the tile (0: nothing to do)
+    int np, nt;        // prefix / tree key tiles of the request (after the mode bits)
+    int j_begin, n_tiles;
+    int n_chunks;      // non-empty chunks of the group = CTAs that arrive at the group counter
+    int group;         // (b*Hkv + g)*n_mt + tile
+    int T, L;
+};
+
+struct TileInfo {
+    int valid;      // keys of the tile that exist (1..128)
+    int row;        // first row of the tile in its tensor map
+    bool tree;      // tree tile (ancestor mask applies), else prefix tile
+    int tt;         // tree tile index (tree tiles only)
+    int j;          // key tile index within the request (prefix tiles first)
+};
+
+__device__ __forceinline__ float4 ld_cg_f4(const float* p) {
+    float4 v;
+    asm volatile("ld.global.cg.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+    return v;
+}
+
+// -------------------------------------------------------------------------------------------------
+// Cascade merge of one group's rows (log-sum-exp state merge):
+//   LSE = log sum_p e^{LSE_p};  O = sum_p e^{LSE_p - LSE} O_p   over the group's chunk states.
+// CTA `chunk` of the group's n_chunks CTAs takes a contiguous range of the tile's rows.  The partial
+// states were written by other SMs and published with a release; they are read at L2 (ld.global.cg),
+// a row of a state per warp instruction (512 contiguous bytes), three rows of up to eight states in
+// flight per warp.  `wts` is shared memory for the normalised weights [state][row].
+__device__ __forceinline__ void merge_rows(const AttnPlan& pl, const AttnArgs& a, float* dbg_rows, const Work& wk,
+                                           float* wts, int warp, int lane) {
+    const int G = pl.G;
+    const int nc = wk.n_chunks;  // <= 64 states
+    const size_t grp0 = (size_t)wk.group * pl.grp_rows;
+    const int r0 = wk.rows * wk.chunk / nc, r1 = wk.rows * (wk.chunk + 1) / nc;
+    const int nrows = r1 - r0;  // <= 128
+    if (nrows <= 0) return;
+    const int tid = warp * 32 + lane;
+    auto out_row = [&](int r) {  // index of query row r0 + r of the tile in out / lse: [b][t][h]
+        const int ra = wk.row_base + r0 + r, t = ra / G;
+        return ((size_t)wk.b * pl.T_cap + t) * pl.Hq + wk.g * G + (ra - t * G);
+    };
+    // step 1, one thread per row: LSE = m + log sum_p e^{LSE_p - m}; weights e^{LSE_p - LSE} to shared
+    // memory (a state without any key: weight 0)
+    if (tid < nrows) {
+        const float* lp = a.part_lse + grp0 + r0 + tid;
+        float m = -INFINITY;
+        for (int i = 0; i < nc; ++i) {
+            const float v = __ldcg(lp + (size_t)i * kTileM);
+            wts[i * kTileM + tid] = v;
+            m = fmaxf(m, v);
+        }
+        float wsum = 0.f;
+        for (int i = 0; i < nc; ++i) {
+            const float v = wts[i * kTileM + tid];
+            const float wv = v == -INFINITY ? 0.f : __expf(v - m);
+            wsum += wv;
+            wts[i * kTileM + tid] = wv;
+        }
+        const float inv = wsum > 0.f ? 1.f / wsum : 0.f;  // no key at all (L = 0, prefix-only mode): O = 0, LSE = -inf
+        for (int i = 0; i < nc; ++i) wts[i * kTileM + tid] *= inv;
+        const float lse = wsum > 0.f ? m + logf(wsum) : -INFINITY;
+        const size_t orow = out_row(tid);
+        if (dbg_rows) dbg_rows[orow * (kD + 1) + kD] = lse;
+        else if (a.lse) a.lse[orow] = lse;
+    }
+    named_bar_sync(9, 256);
+    // step 2, one warp per row, lane = 16-byte chunk: O = sum_p weight_p O_p.  States without any key hold
+    // zeros (their CTA wrote them), so no value needs guarding.
+    constexpr int kRB = 3, kSB = 8;
+    for (int rb = warp * kRB; rb < nrows; rb += 8 * kRB) {
+        float4 acc[kRB];
+#pragma unroll
+        for (int u = 0; u < kRB; ++u) acc[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int s0 = 0; s0 < nc; s0 += kSB) {
+            float4 v[kRB][kSB];
+#pragma unroll
+            for (int u = 0; u < kRB; ++u)
+#pragma unroll
+                for (int i = 0; i < kSB; ++i)
+                    if (rb + u < nrows && s0 + i < nc)
+                        v[u][i] = ld_cg_f4(a.part_o + (grp0 + (size_t)(s0 + i) * kTileM + r0 + rb + u) * kD + lane * 4);
+#pragma unroll
+            for (int u = 0; u < kRB; ++u)
+#pragma unroll
+                for (int i = 0; i < kSB; ++i)
+                    if (rb + u < nrows && s0 + i < nc) {
+                        const float wv = wts[(s0 + i) * kTileM + rb + u];
+                        acc[u].x += wv * v[u][i].x; acc[u].y += wv * v[u][i].y;
+                        acc[u].z += wv * v[u][i].z; acc[u].w += wv * v[u][i].w;
+                    }
+        }
+#pragma unroll
+        for (int u = 0; u < kRB; ++u) {
+            if (rb + u >= nrows) continue;
+            const size_t orow = out_row(rb + u);
+            if (dbg_rows) {  // fp32 state for tests
+                float* d0 = dbg_rows + orow * (kD + 1) + lane * 4;
+                d0[0] = acc[u].x; d0[1] = acc[u].y; d0[2] = acc[u].z; d0[3] = acc[u].w;
+                continue;
+            }
+            uint2 pk;
+            pk.x = pack2_bf16(acc[u].x, acc[u].y);
+            pk.y = pack2_bf16(acc[u].z, acc[u].w);
+            *reinterpret_cast<uint2*>(a.out + orow * kD + lane * 4) = pk;
+        }
+    }
+}
+
+// mode bits: 1 = include the prefix tiles, 2 = include the tree tiles (3 = the whole cascade).
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
+attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
+                   const __grid_constant__ CUtensorMap tm_v, const __grid_constant__ CUtensorMap tm_tk,
+                   const __grid_constant__ CUtensorMap tm_tv, AttnPlan pl, AttnArgs a, int mode, float* dbg_rows) {
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    const uint32_t smem_raw_u32 = (uint32_t)__cvta_generic_to_shared(smem_raw);
+    const uint32_t smem = (smem_raw_u32 + 1023u) & ~1023u;  // 128B swizzle atoms need 1024 B alignment
+    if (smem - smem_raw_u32 + kSmemUsed > kSmemBytes) __trap();
+    unsigned char* smem_gen = smem_raw + (smem - smem_raw_u32);
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const uint32_t bar0 = smem + kOffBar;
+    auto bar = [&](uint32_t i) { return bar0 + 8u * i; };
+    volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(smem_gen + kOffBar + 8u * kTmemSlot);
+
+    // static part of the work decode (no global memory): which cluster kind this CTA belongs to
+    const int n_pairs = pl.n_mt >> 1;
+    const int pair_ctas = n_pairs * 2 * pl.chunks_a;
+    const bool pair = (int)blockIdx.x < pair_ctas;  // cluster of M tiles (2p, 2p+1) over one chunk
+
+    // ---- prologue that touches no global memory (overlaps the preceding kernel's tail under PDL) ----
+    if (warp == 8 && lane == 0) {
+        mbar_init(bar(kBarQFull), 1);
+        for (int i = 0; i < kRingK; ++i) {
+            mbar_init(bar(kBarKFull + i), 1);
+            mbar_init(bar(kBarKEmpty + i), pair ? 2 : 1);  // released by both CTAs of a pair cluster
+        }
+        for (int i = 0; i < kRingV; ++i) {
+            mbar_init(bar(kBarVFull + i), 1);
+            mbar_init(bar(kBarVEmpty + i), pair ? 2 : 1);
+        }
+        for (int s = 0; s < 2; ++s) {
+            mbar_init(bar(kBarSFull + s), 1);
+            mbar_init(bar(kBarSFree + s), 4);  // one elected arrival per warp of the owning team
+            for (int q = 0; q < 4; ++q) mbar_init(bar(kBarPFull + 4 * s + q), 4);
+            mbar_init(bar(kBarPFree + s), 1);
+            mbar_init(bar(kBarVFix + s), 1);
+        }
+        mbar_init(bar(kBarAllDone), 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        tma_prefetch_desc(&tm_q);
+        tma_prefetch_desc(&tm_k);
+        tma_prefetch_desc(&tm_v);
+        tma_prefetch_desc(&tm_tk);
+        tma_prefetch_desc(&tm_tv);
+    }
+    if (warp == 10) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(bar(kTmemSlot)),
+                     "r"(kTmemCols)
+                     : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = *tmem_slot;
+    if (pair) cluster_sync_all();  // the peer's barriers are initialised before anything remote reaches them
+    pdl_launch_dependents();  // the next kernel may begin its own prologue as SMs free up
+    pdl_wait();               // everything before this kernel in the stream is complete and visible
+
+    // ---- this CTA's work ----
+    Work wk;
+    {
+        const int G = pl.G;
+        wk.g = blockIdx.y;
+        wk.b = blockIdx.z;
+        int x = blockIdx.x, n_static;
+        bool pad = false;
+        if (pair) {
+            const int p = x / (2 * pl.chunks_a), r = x - p * 2 * pl.chunks_a;
+            wk.chunk = r >> 1; wk.rank = r & 1; wk.tile = 2 * p + wk.rank; n_static = pl.chunks_a;
+        } else {
+            x -= pair_ctas;
+            wk.chunk = x; wk.rank = x & 1; wk.tile = pl.n_mt - 1; n_static = pl.chunks_b;
+            pad = x >= pl.chunks_b;  // the odd tile's chunk count rounded up to whole clusters
+        }
+        wk.T = a.tree_len[wk.b];
+        wk.L = a.ctx_len[wk.b];
+        const int rows_valid = wk.T * G;
+        wk.row_base = wk.tile * kTileM;
+        wk.rows = pad ? 0 : max(0, min(kTileM, rows_valid - wk.row_base));
+        // a pair shares its key tiles when both M tiles hold rows (a short tree leaves the odd tile empty)
+        wk.share = pair && rows_valid > (wk.tile | 1) * kTileM;
+        wk.group = (wk.b * pl.Hkv + wk.g) * pl.n_mt + wk.tile;
+        wk.np = (mode & 1) ? (wk.L + kTileN - 1) / kTileN : 0;
+        wk.nt = (mode & 2) ? (wk.T + kTileN - 1) / kTileN : 0;
+        const int nk = wk.np + wk.nt;
+        const int tps = max(max(1, pl.tps_min), (nk + n_static - 1) / n_static);
+        wk.n_chunks = max(1, (nk + tps - 1) / tps);  // chunk 0 always takes part (nk = 0: state (0, -inf))
+        wk.j_begin = wk.chunk * tps;
+        wk.n_tiles = max(0, min(nk, wk.j_begin + tps) - wk.j_begin);
+    }
+    // M tiles past the tree's rows, and chunks past the request's key tiles, leave at once:
+    // nobody waits for them (n_chunks counts the non-empty chunks only)
+    const bool idle = wk.rows == 0 || wk.chunk >= wk.n_chunks;
+    const int kv_row0 = a.kv_indptr ? a.kv_indptr[wk.b] : 0;
+    auto tile_info = [&](int jj) {
+        const int j = wk.j_begin + jj;
+        TileInfo ti;
+        ti.j = j;
+        ti.tree = j >= wk.np;
+        ti.tt = j - wk.np;
+        ti.valid = ti.tree ? min(kTileN, wk.T - ti.tt * kTileN) : min(kTileN, wk.L - j * kTileN);
+        ti.row = ti.tree ? wk.b * pl.T_cap + ti.tt * kTileN : kv_row0 + j * kTileN;  // (contiguous KV)
+        return ti;
+    };
+    const uint16_t mc_mask = wk.share ? 3 : (uint16_t)(1u << (blockIdx.x & 1));
+
+    // the control warpgroup hands registers to the two softmax warpgroups (one instruction per warpgroup)
+    if (warp >= 8) {
+      asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsControl));
+      if (idle) {
+        // fall through to the TMEM release
+      } else if (warp == 8 || warp == 9) {
+        // ===== K producer (warp 8, also loads Q) and V producer (warp 9): one ring of three tiles each.
+        // Contiguous KV: lane 0 issues one 32 KiB box per tile.  Paged KV (page = 16 keys): a 128-key
+        // tile is 8 pages; lane 2p+hi issues the 2 KiB box (page p, d half hi), so a tile is 16 loads in
+        // flight at once; only the ceil(valid/16) pages that exist are loaded (the MMAs never read past
+        // ceil16(valid) keys); the page ids of the next tile are fetched one tile ahead.
+        // Sharing pair: both CTAs wait for their slot (released by BOTH CTAs' MMAs) and arm their own full
+        // barrier; rank 0 issues every K load, rank 1 every V load, multicast into both CTAs' rings.
+        // The V producer also zeroes the V rows behind a ragged tile end in its own CTA's copy: the P.V MMA
+        // runs over ceil16(valid) keys, rows valid..ceil16(valid)-1 belong to nobody (next request, tree
+        // padding), are multiplied by P = 0 exactly and must not hold NaN/Inf.  A row is 2 x 128 B (d
+        // halves); the 128B swizzle permutes 16-byte chunks inside a row's 128 B only. =====
+        const bool is_v = warp == 9;
+        const bool paged = pl.page_size > 0;
+        const bool issuer = !wk.share || wk.rank == (is_v ? 1 : 0);
+        const int ring = is_v ? kRingV : kRingK;
+        const uint32_t ring_off = is_v ? kOffV : kOffK;
+        const uint32_t bar_full = is_v ? kBarVFull : kBarKFull, bar_empty = is_v ? kBarVEmpty : kBarKEmpty;
+        auto page_of = [&](int jj) {
+            int pg = 0;
+            if (paged && issuer && jj < wk.n_tiles) {
+                const TileInfo t2 = tile_info(jj);
+                const int p = lane >> 1;
+                if (!t2.tree && lane < 16 && p * 16 < t2.valid) pg = __ldg(a.kv_indices + kv_row0 + t2.j * 8 + p);
+            }
+            return pg;
+        };
+        if (!is_v && lane == 0) {  // Q first: one box = the 128-row query tile of this kv head
+            const int t0 = wk.b * pl.T_cap + wk.row_base / pl.G;
+            mbar_expect_tx(bar(kBarQFull), kQTileBytes);
+            tma_load_5d(smem + kOffQ, &tm_q, bar(kBarQFull), 0, 0, t0, 0, wk.g, kEvictLast);
+        }
+        int page_cur = page_of(0);
+        int n_ragged = 0;
+        for (int jj = 0; jj < wk.n_tiles; ++jj) {
+            const TileInfo ti = tile_info(jj);
+            const int page_next = page_of(jj + 1);
+            const int i = jj % ring;
+            const uint32_t dst = smem + ring_off + i * kKvTileBytes;
+            const uint32_t fb = bar(bar_full + i);
+            const bool by_page = paged && !ti.tree;
+            const int n_pages = (ti.valid + 15) >> 4;
+            if (lane == 0) {
+                mbar_wait(bar(bar_empty + i), ((jj / ring) & 1) ^ 1);
+                mbar_expect_tx(fb, by_page ? (uint32_t)n_pages * 4096u : kKvTileBytes);
+            }
+            __syncwarp();
+            if (issuer) {
+                if (by_page) {
+                    if (lane < 2 * n_pages) {
+                        const uint32_t d2 = dst + (uint32_t)(lane & 1) * (kKvTileBytes / 2) + (uint32_t)(lane >> 1) * 2048u;
+                        if (wk.share)
+                            tma_load_5d_mc(d2, is_v ? &tm_v : &tm_k, fb, 0, 0, lane & 1, wk.g, page_cur, mc_mask, kEvictNormal);
+                        else
+                            tma_load_5d(d2, is_v ? &tm_v : &tm_k, fb, 0, 0, lane & 1, wk.g, page_cur, kEvictNormal);
+                    }
+                } else if (lane == 0) {
+                    const CUtensorMap* tm = ti.tree ? (is_v ? &tm_tv : &tm_tk) : (is_v ? &tm_v : &tm_k);
+                    const uint64_t hint = ti.tree ? kEvictLast : kEvictNormal;
+                    if (wk.share) tma_load_4d_mc(dst, tm, fb, 0, ti.row, 0, wk.g, mc_mask, hint);
+                    else tma_load_4d(dst, tm, fb, 0, ti.row, 0, wk.g, hint);
+                }
+            }
+            if (is_v && (ti.valid & 15) != 0) {
+                mbar_wait(fb, (jj / ring) & 1);  // this fill has landed (every lane observes it)
+                const int n_rows = ((ti.valid + 15) & ~15) - ti.valid;
+                for (int e = lane; e < n_rows * 16; e += 32) {  // 16 x 16 B per row
+                    const int row = ti.valid + (e >> 4), c16 = e & 15;
+                    const uint32_t addr = dst + (uint32_t)(c16 >> 3) * (kKvTileBytes / 2) + (uint32_t)row * 128u +
+                                          (uint32_t)(c16 & 7) * 16u;
+                    asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(addr), "r"(0u) : "memory");
+                }
+                fence_async_smem();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar(kBarVFix + n_ragged));
+                ++n_ragged;
+            }
+            __syncwarp();
+            page_cur = page_next;
+        }
+      } else if (warp == 10) {
+        // ===== MMA issuer: one elected thread walks the unit sequence.  Q.K^T of unit n+2 goes out as soon
+        // as the owning team has read S_n (S and P are separate TMEM columns), P.V of unit n as its P pieces
+        // arrive; the tensor pipe executes them in this order.  A ring slot is released by the commit behind
+        // its last reader (to both CTAs of a sharing pair). =====
+        if (elect_one()) {
+            const uint64_t qd = smem_desc(smem + kOffQ, 16, 1024);
+            const uint32_t od = tmem;
+            const int N = wk.n_tiles;
+            auto release = [&](uint32_t b) {
+                if (wk.share) tc_commit_mc(b, 3);
+                else { tc_commit(b); if (pair) tc_commit(b); }  // a pair cluster's barriers count two releases
+            };
+            auto issue_qk = [&](int n) {
+                const int i = n % kRingK, s = n & 1;
+                mbar_wait(bar(kBarKFull + i), (n / kRingK) & 1);
+                const int tile_n = (tile_info(n).valid + 15) & ~15;  // MMA N (multiple of 16)
+                const uint64_t kd = smem_desc(smem + kOffK + i * kKvTileBytes, 16, 1024);
+                const uint32_t id_qk = idesc(kTileM, (uint32_t)tile_n, 0);
+                const uint32_t sd = tmem + kTmemS + s * kTileN;
+                tc_fence_after();
+#pragma unroll
+                for (int kk = 0; kk < kD / 16; ++kk) {
+                    const uint64_t off = (uint64_t)(((kk >> 2) * (kQTileBytes / 2) + (kk & 3) * 32) >> 4);
+                    umma_ss(sd, qd + off, kd + off, id_qk, kk > 0);
+                }
+                tc_commit(bar(kBarSFull + s));
+                release(bar(kBarKEmpty + i));  // K_n is free once this Q.K^T has completed
+            };
+            mbar_wait(bar(kBarQFull), 0);  // (also with N = 0: the CTA must not leave with the load in flight)
+            if (N > 0) issue_qk(0);
+            if (N > 1) issue_qk(1);
+            uint32_t n_ragged = 0;
+            for (int n = 0; n < N; ++n) {
+                const int s = n & 1, par = (n >> 1) & 1;
+                if (n + 2 < N) {
+                    mbar_wait(bar(kBarSFree + s), par);  // S_n is in the team's registers
+                    issue_qk(n + 2);
+                }
+                const int valid = tile_info(n).valid;
+                const int ksteps = ((valid + 15) & ~15) >> 4;  // K extent of P.V in 16-key steps
+                const int vi = n % kRingV;
+                mbar_wait(bar(kBarVFull + vi), (n / kRingV) & 1);
+                if (valid & 15) mbar_wait(bar(kBarVFix + n_ragged++), 0);
+                const uint64_t vd = smem_desc(smem + kOffV + vi * kKvTileBytes, kKvTileBytes / 2, 1024);
+                const uint32_t pd = tmem + kTmemP + s * (kTileN / 2);
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    // every piece is awaited, also the ones past a ragged tile's end that feed no MMA (the
+                    // barrier phases stay in step)
+                    mbar_wait(bar(kBarPFull + 4 * s + q), par);
+                    tc_fence_after();
+#pragma unroll
+                    for (int ks = 2 * q; ks < 2 * q + 2; ++ks)
+                        if (ks < ksteps) umma_ts(od, pd + ks * 8, vd + (uint64_t)(ks * (2048 >> 4)), kIdescPV, (n > 0) | ks);
+                }
+                tc_commit(bar(kBarPFree + s));
+                release(bar(kBarVEmpty + vi));  // V_n is free once these P.V pieces have completed
+            }
+            tc_commit(bar(kBarAllDone));
+        }
+      }
+    } else {
+      asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegsSoftmax));
+      if (!idle) {
+        // ===== softmax: team A (warps 0..3) owns the even units, team B (warps 4..7) the odd ones; thread
+        // (w, lane) of either team owns query row w*32 + lane (TMEM lane) and a whole 128-key score row.
+        // While one team is in its exponentials the other loads, takes maxima, packs and stores. =====
+        const int g = warp >> 2;       // team
+        const int w = warp & 3;
+        const int rl = w * 32 + lane;  // row within the tile
+        const uint32_t lane_addr = (uint32_t)(w * 32) << 16;
+        const float c2 = pl.sm_scale * kLog2e;
+        const float thr = kRescaleThreshold / c2;  // in raw score units
+        float* xm = reinterpret_cast<float*>(smem_gen + kOffX);  // [team][row]: reference maximum after the team's last unit
+        const bool warp_active = w * 32 < wk.rows;
+        const int N = wk.n_tiles;
+        float m_mine = -INFINITY;  // the reference this thread's row sum is relative to
+        float l_mine = 0.f;
+        const int t_node = min((wk.row_base + rl) / pl.G, wk.T - 1);
+        const uint32_t* mrow = a.mask + ((size_t)wk.b * pl.T_cap + t_node) * pl.W;
+        for (int n = g; n < N; n += 2) {
+            const int s = g, par = (n >> 1) & 1;
+            const TileInfo ti = tile_info(n);
+            const uint32_t sbuf = tmem + kTmemS + s * kTileN + lane_addr;
+            const uint32_t pbuf = tmem + kTmemP + s * (kTileN / 2) + lane_addr;
+            mbar_wait(bar(kBarSFull + s), par);
+            if (!warp_active) {  // a warp without rows only keeps the barrier phases in step
+                if (lane == 0) {
+                    mbar_arrive(bar(kBarSFree + s));
+                    if (n >= 2) mbar_wait(bar(kBarPFree + s), par ^ 1);
+                    for (int q = 0; q < 4; ++q) mbar_arrive(bar(kBarPFull + 4 * s + q));
+                }
+                __syncwarp();
+                continue;
+            }
+            uint32_t sv[128];
+            tc_fence_after();
+            D2SD_TMEM_LD32(sbuf, sv, 0);
+            D2SD_TMEM_LD32(sbuf + 32, sv, 32);
+            D2SD_TMEM_LD32(sbuf + 64, sv, 64);
+            D2SD_TMEM_LD32(sbuf + 96, sv, 96);
+            tmem_wait_ld();
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar(kBarSFree + s));  // Q.K^T of unit n+2 may overwrite S now
+            if (ti.tree || ti.valid < kTileN) {
+                // keys past the tile's end, and (tree tiles) keys that are not ancestors-or-self of this
+                // row's node: the tile's 128 mask bits -> -inf
+                uint32_t mw[4] = {0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu};
+                if (ti.tree) {
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) mw[u] = ti.tt * 4 + u < pl.W ? mrow[ti.tt * 4 + u] : 0u;
+                }
+#pragma unroll
+                for (int c = 0; c < 128; ++c) {
+                    const uint32_t bit = (mw[c >> 5] >> (c & 31)) & 1u;
+                    if (c >= ti.valid || !bit) sv[c] = 0xFF800000u;
+                }
+            }
+            float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;
+#pragma unroll
+            for (int c = 0; c < 128; c += 4) {
+                mx0 = fmaxf(mx0, __uint_as_float(sv[c]));
+                mx1 = fmaxf(mx1, __uint_as_float(sv[c + 1]));
+                mx2 = fmaxf(mx2, __uint_as_float(sv[c + 2]));
+                mx3 = fmaxf(mx3, __uint_as_float(sv[c + 3]));
+            }
+            const float mx = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
+            // reference hand-off: m_ref(n-1) from the other team (ordered by the warp pair's named barrier),
+            // lazy raise, m_ref(n) to the other team
+            float m_prev = -INFINITY;
+            if (n > 0) {
+                named_bar_sync(1 + 4 * (g ^ 1) + w, 64);
+                m_prev = xm[(g ^ 1) * kTileM + rl];
+            }
+            const bool need = n > 0 && mx > m_prev + thr;
+            const float m_new = n == 0 ? mx : (need ? mx : m_prev);
+            if (n + 1 < N) {
+                xm[g * kTileM + rl] = m_new;
+                named_bar_arrive(1 + 4 * g + w, 64);
+            }
+            if (m_new != m_mine) {  // this thread's own row sum follows the reference
+                l_mine *= m_mine == -INFINITY ? 0.f : ex2((m_mine - m_new) * c2);
+                m_mine = m_new;
+            }
+            if (__any_sync(0xffffffffu, need)) {
+                // O holds units < n relative to m_prev: wait for P.V of unit n-1 (the other buffer's), rescale
+                // this row.  P.V of unit n cannot start before this thread releases P_n below.
+                mbar_wait(bar(kBarPFree + (s ^ 1)), ((n - 1) >> 1) & 1);
+                tc_fence_after();
+                const float alpha = need ? (m_prev == -INFINITY ? 0.f : ex2((m_prev - m_new) * c2)) : 1.f;
+#pragma unroll 1
+                for (int c0 = 0; c0 < kD; c0 += 32) {
+                    uint32_t o[32];
+                    D2SD_TMEM_LD32(tmem + lane_addr + c0, o, 0);
+                    tmem_wait_ld();
+#pragma unroll
+                    for (int c = 0; c < 32; ++c) o[c] = __float_as_uint(__uint_as_float(o[c]) * alpha);
+                    D2SD_TMEM_ST32(tmem + lane_addr + c0, o, 0);
+                }
+                tmem_wait_st();
+                tc_fence_before();
+            }
+            // the P buffer is free once P.V of unit n-2 has completed
+            if (n >= 2) mbar_wait(bar(kBarPFree + s), par ^ 1);
+            // a row with every key so far masked has m_ref = -inf: exp2(-inf - 0) = 0, not NaN
+            const float ms = m_new == -INFINITY ? 0.f : m_new * c2;
+            float sum0 = 0.f, sum1 = 0.f;
+            // P[128 x 128] bf16 = 64 TMEM columns, written and released in four 32-key pieces; the store of a
+            // piece is only waited for after the next piece's exponentials
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                float ev[32];
+#pragma unroll
+                for (int c = 0; c < 32; ++c) ev[c] = ex2_ordered(__uint_as_float(sv[q * 32 + c]) * c2 - ms);
+                if (q > 0) {
+                    tmem_wait_st();
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(bar(kBarPFull + 4 * s + q - 1));
+                }
+                uint32_t p[16];
+                float t0 = 0.f, t1 = 0.f, t2 = 0.f, t3 = 0.f;
+#pragma unroll
+                for (int c = 0; c < 16; c += 2) {
+                    t0 += ev[2 * c]; t1 += ev[2 * c + 1]; t2 += ev[2 * c + 2]; t3 += ev[2 * c + 3];
+                    p[c] = pack2_bf16(ev[2 * c], ev[2 * c + 1]);
+                    p[c + 1] = pack2_bf16(ev[2 * c + 2], ev[2 * c + 3]);
+                }
+                sum0 += t0 + t1;
+                sum1 += t2 + t3;
+                D2SD_TMEM_ST16(pbuf + q * 16, p);
+            }
+            l_mine += sum0 + sum1;
+            tmem_wait_st();
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar(kBarPFull + 4 * s + 3));
+        }
+        // ---- epilogue: the two teams' row sums meet at the final reference; the normalised state leaves the
+        // CTA straight from registers through a per-warp transpose in shared memory (the rings are free):
+        // thread (team g, w, lane) holds columns 64g..64g+63 of row w*32+lane, the warp writes them as 256-byte
+        // runs.  A group with a single chunk writes its rows to `out` directly: no exchange at all. ----
+        if (warp_active && N > 0 && ((N - 1) & 1) == g) xm[g * kTileM + rl] = m_mine;  // owner of the last unit
+        mbar_wait(bar(kBarAllDone), 0);  // every MMA done: O is final, the rings are free
+        named_bar_sync(9, 256);
+        const float m_fin = N > 0 ? xm[((N - 1) & 1) * kTileM + rl] : -INFINITY;
+        if (m_fin != m_mine) l_mine *= m_mine == -INFINITY ? 0.f : ex2((m_mine - m_fin) * c2);
+        float* xl = reinterpret_cast<float*>(smem_gen + kOffXL);
+        xl[g * kTileM + rl] = l_mine;
+        named_bar_sync(10, 256);
+        const float l_tot = l_mine + xl[(g ^ 1) * kTileM + rl];
+        const float inv = l_tot > 0.f ? 1.f / l_tot : 0.f;  // l = 0: every key of the chunk masked, or no key at all
+        const float lse_v = l_tot > 0.f ? m_fin * pl.sm_scale + logf(l_tot) : -INFINITY;
+        const bool direct = wk.n_chunks == 1;
+        const bool row_ok = rl < wk.rows;
+        const size_t prow0 = (size_t)wk.group * pl.grp_rows + (size_t)wk.chunk * kTileM;
+        if (warp_active) {
+            const uint32_t region = smem + kOffK + (uint32_t)warp * 8192u;  // [32 rows][256 B], 16-byte chunks XOR-swizzled
+            tc_fence_after();
+#pragma unroll
+            for (int c0 = 0; c0 < 64; c0 += 32) {
+                uint32_t ov[32];
+                if (N > 0) {
+                    D2SD_TMEM_LD32(tmem + lane_addr + g * 64 + c0, ov, 0);
+                    tmem_wait_ld();
+                }
+#pragma unroll
+                for (int c = 0; c < 32; c += 4) {
+                    const uint32_t chunk = (uint32_t)((c0 + c) >> 2) ^ ((uint32_t)lane & 15u);
+                    float f0 = 0.f, f1 = 0.f, f2 = 0.f, f3 = 0.f;
+                    if (N > 0) {
+                        f0 = __uint_as_float(ov[c]) * inv; f1 = __uint_as_float(ov[c + 1]) * inv;
+                        f2 = __uint_as_float(ov[c + 2]) * inv; f3 = __uint_as_float(ov[c + 3]) * inv;
+                    }
+                    asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(region + (uint32_t)lane * 256u + chunk * 16u),
+                                 "f"(f0), "f"(f1), "f"(f2), "f"(f3)
+                                 : "memory");
+                }
+            }
+            __syncwarp();
+            const int G = pl.G;
+#pragma unroll 4
+            for (int it = 0; it < 16; ++it) {
+                const int row = it * 2 + (lane >> 4), ck = lane & 15;
+                float4 v;
+                asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];"
+                             : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
+                             : "r"(region + (uint32_t)row * 256u + (uint32_t)((ck ^ (row & 15)) * 16)));
+                const int r = w * 32 + row;  // row of the tile
+                if (r >= wk.rows) continue;
+                const int col = g * 64 + ck * 4;
+                if (!direct) {
+                    *reinterpret_cast<float4*>(a.part_o + (prow0 + r) * kD + col) = v;
+                } else {
+                    const int ra = wk.row_base + r, t = ra / G;
+                    const size_t orow = ((size_t)wk.b * pl.T_cap + t) * pl.Hq + wk.g * G + (ra - t * G);
+                    if (dbg_rows) {
+                        float* d0 = dbg_rows + orow * (kD + 1) + col;
+                        d0[0] = v.x; d0[1] = v.y; d0[2] = v.z; d0[3] = v.w;
+                    } else {
+                        uint2 pk;
+                        pk.x = pack2_bf16(v.x, v.y);
+                        pk.y = pack2_bf16(v.z, v.w);
+                        *reinterpret_cast<uint2*>(a.out + orow * kD + col) = pk;
+                    }
+                }
+            }
+            if (g == 0 && row_ok) {
+                if (!direct) {
+                    a.part_lse[prow0 + rl] = lse_v;
+                } else {
+                    const int ra = wk.row_base + rl, t = ra / G;
+                    const size_t orow = ((size_t)wk.b * pl.T_cap + t) * pl.Hq + wk.g * G + (ra - t * G);
+                    if (dbg_rows) dbg_rows[orow * (kD + 1) + kD] = lse_v;
+                    else if (a.lse) a.lse[orow] = lse_v;
+                }
+            }
+        }
+        if (!direct) {
+            // ---- publish this CTA's partial state, wait for the group, merge this CTA's share of rows ----
+            const unsigned expected = (unsigned)wk.n_chunks;
+            unsigned* cnt = a.counters + 2 * wk.group;  // [0] arrivals, [1] done
+            __threadfence();
+            named_bar_sync(9, 256);  // every thread's partial-state writes happen before the leader's release
+            unsigned done_before = 0;
+            int ok = 1;
+            if (warp == 0 && lane == 0) {
+                asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(cnt) : "memory");
+                unsigned seen, spins = 0;
+                do {
+                    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(cnt) : "memory");
+                    if (seen < expected) {
+                        __nanosleep(20);
+                        if (++spins > (1u << 22)) {  // the group never became co-resident: report, do not hang
+                            atomicExch(a.counters + kWsErrorWord, 1u);
+                            ok = 0;
+                            break;
+                        }
+                    }
+                } while (seen < expected);
+                // this CTA is past the wait: count it out now, the round trip hides behind the merge
+                done_before = atomicAdd(cnt + 1, 1u);
+                xl[0] = __int_as_float(ok);
+            }
+            named_bar_sync(10, 256);
+            if (__float_as_int(xl[0]))
+                merge_rows(pl, a, dbg_rows, wk, reinterpret_cast<float*>(smem_gen + kOffV), warp, lane);
+            if (warp == 0 && lane == 0) {
+                if (done_before == expected - 1) {  // last CTA out: everybody is past the wait
+                    cnt[0] = 0;
+                    cnt[1] = 0;
+                }
+            }
+        }
+      }
+    }
+
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 10) {
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(kTmemCols) : "memory");
+    }
+    if (pair) cluster_sync_all();  // no CTA leaves while its peer may still signal its barriers
+}
+
+// ---- host side ----------------------------------------------------------------------------------
+using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_fn() {
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
+            qres == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<EncodeTiledFn>(p);
+    }
+    return fn;
+}
+
+int32_t encode(CUtensorMap* tm, const void* base, int rank, const cuuint64_t* dims, const cuuint64_t* strides,
+               const cuuint32_t* box, const char* what) {
+    EncodeTiledFn fn = encode_fn();
+    if (!fn) return set_error(D2SD_ERR_CUDA, "cuTensorMapEncodeTiled entry point not found");
+    cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+    CUresult r = fn(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, (cuuint32_t)rank, const_cast<void*>(base), dims, strides, box,
+                    estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return set_error(D2SD_ERR_CUDA, "cuTensorMapEncodeTiled(%s) failed with CUresult %d", what, (int)r);
+    return D2SD_OK;
+}
+
+}  // namespace
+
+bool attn_stream_supported(const AttnPlan& pl) {
+    // contiguous or 16-key-paged KV, rows of one query tile must be whole tree nodes (128 % G == 0),
+    // and the tensor-map extents must fit.
+    return (pl.page_size == 0 || pl.page_size == 16) && pl.d == kD && pl.G <= 128 && (128 % pl.G) == 0 &&
+           (int64_t)pl.B * pl.T_cap < (1ll << 31) && pl.kv_rows < (1ll << 31);
+}
+
+int32_t launch_attn_stream(const AttnPlan& pl, const AttnArgs& a, int mode, float* dbg_rows, cudaStream_t s) {
+    static unsigned long long attr_done = 0;
+    if (first_use_on_device(attr_done))
+        D2SD_CHECK_CUDA(cudaFuncSetAttribute(attn_stream_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             (int)kSmemBytes));
+    CUtensorMap tm_q, tm_k, tm_v, tm_tk, tm_tv;
+    {   // Q [B*T_cap, Hq, d] viewed as (d_lo 64, hh G, t B*T_cap, d_hi 2, g Hkv): one box = one 128-row query tile
+        const cuuint64_t dims[5] = {64, (cuuint64_t)pl.G, (cuuint64_t)pl.B * pl.T_cap, 2, (cuuint64_t)pl.Hkv};
+        const cuuint64_t strides[4] = {(cuuint64_t)kD * 2, (cuuint64_t)pl.Hq * kD * 2, 128, (cuuint64_t)pl.G * kD * 2};
+        const cuuint32_t box[5] = {64, (cuuint32_t)pl.G, (cuuint32_t)(kTileM / pl.G), 2, 1};
+        if (int32_t st = encode(&tm_q, a.q, 5, dims, strides, box, "q")) return st;
+    }
+    {   // K/V [rows, Hkv, d] viewed as (d_lo 64, row, d_hi 2, g): one box = one 128-key tile.  Rows past the
+        // end of the tensor are zero-filled by TMA; the kernel masks every key past a tile's valid count.
+        const cuuint64_t strides[3] = {(cuuint64_t)pl.Hkv * kD * 2, 128, (cuuint64_t)kD * 2};
+        const cuuint32_t box[4] = {64, kTileN, 2, 1};
+        const cuuint64_t tdims[4] = {64, (cuuint64_t)pl.B * pl.T_cap, 2, (cuuint64_t)pl.Hkv};
+        if (int32_t st = encode(&tm_tk, a.tree_k, 4, tdims, strides, box, "tree_k")) return st;
+        if (int32_t st = encode(&tm_tv, a.tree_v, 4, tdims, strides, box, "tree_v")) return st;
+        if (pl.kv_rows > 0 && a.k_cache && a.v_cache && pl.page_size > 0) {
+            // paged pool [P, 16, Hkv, d] viewed as (d_lo 64, slot 16, d_hi 2, g, page): one box = one d half
+            // of one page of one kv head (2 KiB); 16 boxes make a 128-key tile in the same shared-memory
+            // image as a contiguous tile (the 128B swizzle is a function of the shared-memory address)
+            const cuuint64_t pdims[5] = {64, 16, 2, (cuuint64_t)pl.Hkv, (cuuint64_t)(pl.kv_rows / 16)};
+            const cuuint64_t pstrides[4] = {(cuuint64_t)pl.Hkv * kD * 2, 128, (cuuint64_t)kD * 2,
+                                            (cuuint64_t)16 * pl.Hkv * kD * 2};
+            const cuuint32_t pbox[5] = {64, 16, 1, 1, 1};
+            if (int32_t st = encode(&tm_k, a.k_cache, 5, pdims, pstrides, pbox, "k_pool")) return st;
+            if (int32_t st = encode(&tm_v, a.v_cache, 5, pdims, pstrides, pbox, "v_pool")) return st;
+        } else if (pl.kv_rows > 0 && a.k_cache && a.v_cache) {
+            const cuuint64_t dims[4] = {64, (cuuint64_t)pl.kv_rows, 2, (cuuint64_t)pl.Hkv};
+            if (int32_t st = encode(&tm_k, a.k_cache, 4, dims, strides, box, "k_cache")) return st;
+            if (int32_t st = encode(&tm_v, a.v_cache, 4, dims, strides, box, "v_cache")) return st;
+        } else {  // no committed prefix at all (max_ctx_len == 0): the maps are never used
+            tm_k = tm_tk;
+            tm_v = tm_tv;
+        }
+    }
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((pl.n_mt >> 1) * 2 * pl.chunks_a + (pl.n_mt & 1) * ((pl.chunks_b + 1) & ~1), pl.Hkv, pl.B);
+    cfg.blockDim = dim3(kThreads);
+    cfg.dynamicSmemBytes = kSmemBytes;
+    cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;  // PDL: see the file header
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    D2SD_CHECK_CUDA(cudaLaunchKernelEx(&cfg, attn_stream_kernel, tm_q, tm_k, tm_v, tm_tk, tm_tv, pl, a, mode, dbg_rows));
+    D2SD_CHECK_LAUNCH("attn_stream_kernel");
+    return D2SD_OK;
+}
+
+
+}  // namespace d2sd

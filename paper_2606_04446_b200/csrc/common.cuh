@@ -58,6 +58,7 @@ inline bool first_use_on_device(unsigned long long& done_mask) {
     return true;
 }
 constexpr size_t kWsHeaderBytes = 1u << 20;  // fixed-size head of the attention workspace (group counters)
+constexpr unsigned kWsErrorWord = (1u << 20) / 4 - 2;  // uint32 index in the header: set when a group wait gave up
 
 // ---- stage launchers (defined in the per-stage .cu files) -------------------------------------
 int32_t launch_select(const float* conf, int B, int gamma, int K, int32_t* prefix_len, double* r_out,
@@ -122,6 +123,8 @@ struct AttnPlan {
     bool use_tc;      // tcgen05 prefix pass
     // tcgen05: the query rows (T*G) of one kv head are cut into 128-row tiles; tiles (2p, 2p+1) form
     // "pair item" p, an odd last tile is the "single item".  Item kinds get their own chunk counts.
+    int n_mt;                // 128-row query tiles per (request, kv head), from T_cap
+    bool use_stream;         // the one-tile-per-CTA kernel (attn_stream_sm100.cu): chunks_a per paired tile, chunks_b for an odd last tile
     int n_pair, n_single;    // items per (request, kv head), from T_cap
     int chunks_a, chunks_b;  // CTAs (context chunks) per pair item / per single item
     int tps_min;             // a chunk never holds fewer key tiles than this (unless the request ends)
@@ -145,5 +148,7 @@ int32_t launch_attn_merge(const AttnPlan& pl, const AttnArgs& a, cudaStream_t s)
 // mode: bit 0 = prefix tiles, bit 1 = tree tiles; dbg_rows: fp32 [B][T_cap][Hq][d+1] instead of out/lse
 int32_t launch_attn_cascade_tc(const AttnPlan& pl, const AttnArgs& a, int mode, float* dbg_rows, cudaStream_t s);
 bool attn_cascade_tc_supported(const AttnPlan& pl);
+int32_t launch_attn_stream(const AttnPlan& pl, const AttnArgs& a, int mode, float* dbg_rows, cudaStream_t s);
+bool attn_stream_supported(const AttnPlan& pl);
 
 }  // namespace d2sd
