@@ -309,6 +309,7 @@ int32_t d2sd_cascade_verify_attn(const d2sd_attn_params* p, const void* q, const
     a.lse = lse; a.dbg_state = dbg_state;
     a.part_o = reinterpret_cast<float*>(static_cast<char*>(workspace) + pl.off_o);
     a.part_lse = reinterpret_cast<float*>(static_cast<char*>(workspace) + pl.off_lse);
+    a.part_o16 = reinterpret_cast<__nv_bfloat16*>(static_cast<char*>(workspace) + pl.off_o);
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     const int phases = p->phases ? p->phases : 7;
     const bool do_prefix = phases & 1, do_tree = phases & 2, do_merge = phases & 4;

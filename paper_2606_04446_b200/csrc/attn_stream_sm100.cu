@@ -358,95 +358,116 @@ struct TileInfo {
     int j;          // key tile index within the request (prefix tiles first)
 };
 
-__device__ __forceinline__ float4 ld_cg_f4(const float* p) {
-    float4 v;
-    asm volatile("ld.global.cg.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+__device__ __forceinline__ uint2 ld_cg_u2(const __nv_bfloat16* p) {
+    uint2 v;
+    asm volatile("ld.global.cg.v2.u32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "l"(p));
     return v;
 }
+__device__ __forceinline__ float bf_lo(uint32_t w) { return __uint_as_float(w << 16); }
+__device__ __forceinline__ float bf_hi(uint32_t w) { return __uint_as_float(w & 0xFFFF0000u); }
 
 // -------------------------------------------------------------------------------------------------
 // Cascade merge of one group's rows (log-sum-exp state merge):
 //   LSE = log sum_p e^{LSE_p};  O = sum_p e^{LSE_p - LSE} O_p   over the group's chunk states.
-// CTA `chunk` of the group's n_chunks CTAs takes a contiguous range of the tile's rows.  The partial
-// states were written by other SMs and published with a release; they are read at L2 (ld.global.cg),
-// a row of a state per warp instruction (512 contiguous bytes), three rows of up to eight states in
-// flight per warp.  `wts` is shared memory for the normalised weights [state][row].
+// CTA `chunk` of the group's n_chunks CTAs takes a contiguous range of the tile's rows; a warp takes
+// three rows at a time.  Everything a warp needs for its rows is requested at once -- lane i loads the
+// LSE of state i, every lane loads its 16-byte piece of every state's O row (512 contiguous bytes per
+// warp instruction, up to eight states x three rows in flight) -- so the merge costs one L2 round trip;
+// the weights are reduced with shuffles and never leave the registers.  The partial states were written
+// by other SMs and published with a release; they are read at L2 (ld.global.cg).
 __device__ __forceinline__ void merge_rows(const AttnPlan& pl, const AttnArgs& a, float* dbg_rows, const Work& wk,
-                                           float* wts, int warp, int lane) {
+                                           int warp, int lane) {
     const int G = pl.G;
     const int nc = wk.n_chunks;  // <= 64 states
     const size_t grp0 = (size_t)wk.group * pl.grp_rows;
     const int r0 = wk.rows * wk.chunk / nc, r1 = wk.rows * (wk.chunk + 1) / nc;
     const int nrows = r1 - r0;  // <= 128
-    if (nrows <= 0) return;
-    const int tid = warp * 32 + lane;
-    auto out_row = [&](int r) {  // index of query row r0 + r of the tile in out / lse: [b][t][h]
-        const int ra = wk.row_base + r0 + r, t = ra / G;
-        return ((size_t)wk.b * pl.T_cap + t) * pl.Hq + wk.g * G + (ra - t * G);
-    };
-    // step 1, one thread per row: LSE = m + log sum_p e^{LSE_p - m}; weights e^{LSE_p - LSE} to shared
-    // memory (a state without any key: weight 0)
-    if (tid < nrows) {
-        const float* lp = a.part_lse + grp0 + r0 + tid;
-        float m = -INFINITY;
-        for (int i = 0; i < nc; ++i) {
-            const float v = __ldcg(lp + (size_t)i * kTileM);
-            wts[i * kTileM + tid] = v;
-            m = fmaxf(m, v);
-        }
-        float wsum = 0.f;
-        for (int i = 0; i < nc; ++i) {
-            const float v = wts[i * kTileM + tid];
-            const float wv = v == -INFINITY ? 0.f : __expf(v - m);
-            wsum += wv;
-            wts[i * kTileM + tid] = wv;
-        }
-        const float inv = wsum > 0.f ? 1.f / wsum : 0.f;  // no key at all (L = 0, prefix-only mode): O = 0, LSE = -inf
-        for (int i = 0; i < nc; ++i) wts[i * kTileM + tid] *= inv;
-        const float lse = wsum > 0.f ? m + logf(wsum) : -INFINITY;
-        const size_t orow = out_row(tid);
-        if (dbg_rows) dbg_rows[orow * (kD + 1) + kD] = lse;
-        else if (a.lse) a.lse[orow] = lse;
-    }
-    named_bar_sync(9, 256);
-    // step 2, one warp per row, lane = 16-byte chunk: O = sum_p weight_p O_p.  States without any key hold
-    // zeros (their CTA wrote them), so no value needs guarding.
     constexpr int kRB = 3, kSB = 8;
     for (int rb = warp * kRB; rb < nrows; rb += 8 * kRB) {
+        // lane i holds LSE of states i and i + 32 for each of the three rows
+        float lv[kRB][2];
+#pragma unroll
+        for (int u = 0; u < kRB; ++u)
+#pragma unroll
+            for (int hh = 0; hh < 2; ++hh) {
+                const int i = lane + 32 * hh;
+                lv[u][hh] = (rb + u < nrows && i < nc) ? __ldcg(a.part_lse + grp0 + (size_t)i * kTileM + r0 + rb + u) : -INFINITY;
+            }
+        uint2 v[kRB][kSB];
+#pragma unroll
+        for (int u = 0; u < kRB; ++u)
+#pragma unroll
+            for (int i = 0; i < kSB; ++i)
+                if (rb + u < nrows && i < nc)
+                    v[u][i] = ld_cg_u2(a.part_o16 + (grp0 + (size_t)i * kTileM + r0 + rb + u) * kD + lane * 4);
+        //@T 52
+        float wv[kRB][2], lse[kRB];
+#pragma unroll
+        for (int u = 0; u < kRB; ++u) {
+            float m = fmaxf(lv[u][0], lv[u][1]);
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+            wv[u][0] = lv[u][0] == -INFINITY ? 0.f : __expf(lv[u][0] - m);
+            wv[u][1] = lv[u][1] == -INFINITY ? 0.f : __expf(lv[u][1] - m);
+            float ws = wv[u][0] + wv[u][1];
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) ws += __shfl_xor_sync(0xffffffffu, ws, o);
+            const float inv = ws > 0.f ? 1.f / ws : 0.f;  // no key at all (L = 0, prefix-only mode): O = 0, LSE = -inf
+            wv[u][0] *= inv;
+            wv[u][1] *= inv;
+            lse[u] = ws > 0.f ? m + logf(ws) : -INFINITY;
+        }
+        //@T 53
         float4 acc[kRB];
 #pragma unroll
-        for (int u = 0; u < kRB; ++u) acc[u] = make_float4(0.f, 0.f, 0.f, 0.f);
-        for (int s0 = 0; s0 < nc; s0 += kSB) {
-            float4 v[kRB][kSB];
+        for (int u = 0; u < kRB; ++u) {
+            acc[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+            for (int i = 0; i < kSB; ++i) {
+                const float w1 = __shfl_sync(0xffffffffu, wv[u][0], i);
+                if (rb + u < nrows && i < nc) {  // states without any key hold zeros (their CTA wrote them)
+                    acc[u].x += w1 * bf_lo(v[u][i].x); acc[u].y += w1 * bf_hi(v[u][i].x);
+                    acc[u].z += w1 * bf_lo(v[u][i].y); acc[u].w += w1 * bf_hi(v[u][i].y);
+                }
+            }
+        }
+        //@T 54
+        for (int s0 = kSB; s0 < nc; s0 += kSB) {  // more than eight chunks: further batches of states
 #pragma unroll
             for (int u = 0; u < kRB; ++u)
 #pragma unroll
                 for (int i = 0; i < kSB; ++i)
                     if (rb + u < nrows && s0 + i < nc)
-                        v[u][i] = ld_cg_f4(a.part_o + (grp0 + (size_t)(s0 + i) * kTileM + r0 + rb + u) * kD + lane * 4);
+                        v[u][i] = ld_cg_u2(a.part_o16 + (grp0 + (size_t)(s0 + i) * kTileM + r0 + rb + u) * kD + lane * 4);
 #pragma unroll
             for (int u = 0; u < kRB; ++u)
 #pragma unroll
-                for (int i = 0; i < kSB; ++i)
-                    if (rb + u < nrows && s0 + i < nc) {
-                        const float wv = wts[(s0 + i) * kTileM + rb + u];
-                        acc[u].x += wv * v[u][i].x; acc[u].y += wv * v[u][i].y;
-                        acc[u].z += wv * v[u][i].z; acc[u].w += wv * v[u][i].w;
+                for (int i = 0; i < kSB; ++i) {
+                    const int st = s0 + i;
+                    const float wa = __shfl_sync(0xffffffffu, wv[u][0], st & 31), wb = __shfl_sync(0xffffffffu, wv[u][1], st & 31);
+                    const float w1 = st < 32 ? wa : wb;
+                    if (rb + u < nrows && st < nc) {
+                        acc[u].x += w1 * bf_lo(v[u][i].x); acc[u].y += w1 * bf_hi(v[u][i].x);
+                        acc[u].z += w1 * bf_lo(v[u][i].y); acc[u].w += w1 * bf_hi(v[u][i].y);
                     }
+                }
         }
 #pragma unroll
         for (int u = 0; u < kRB; ++u) {
             if (rb + u >= nrows) continue;
-            const size_t orow = out_row(rb + u);
+            const int ra = wk.row_base + r0 + rb + u, t = ra / G;  // query row of the tile -> out / lse row [b][t][h]
+            const size_t orow = ((size_t)wk.b * pl.T_cap + t) * pl.Hq + wk.g * G + (ra - t * G);
             if (dbg_rows) {  // fp32 state for tests
                 float* d0 = dbg_rows + orow * (kD + 1) + lane * 4;
                 d0[0] = acc[u].x; d0[1] = acc[u].y; d0[2] = acc[u].z; d0[3] = acc[u].w;
+                if (lane == 0) dbg_rows[orow * (kD + 1) + kD] = lse[u];
                 continue;
             }
             uint2 pk;
             pk.x = pack2_bf16(acc[u].x, acc[u].y);
             pk.y = pack2_bf16(acc[u].z, acc[u].w);
             *reinterpret_cast<uint2*>(a.out + orow * kD + lane * 4) = pk;
+            if (lane == 0 && a.lse) a.lse[orow] = lse[u];
         }
     }
 }
@@ -466,6 +487,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
     auto bar = [&](uint32_t i) { return bar0 + 8u * i; };
     volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(smem_gen + kOffBar + 8u * kTmemSlot);
 
+    //@T 0
     // static part of the work decode (no global memory): which cluster kind this CTA belongs to
     const int n_pairs = pl.n_mt >> 1;
     const int pair_ctas = n_pairs * 2 * pl.chunks_a;
@@ -507,9 +529,13 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
-    if (pair) cluster_sync_all();  // the peer's barriers are initialised before anything remote reaches them
+    //@T 1
+    // the peer's barriers must be initialised before anything remote reaches them: arrive now, wait after the
+    // work decode (the peer has long arrived by then)
+    if (pair) asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
     pdl_launch_dependents();  // the next kernel may begin its own prologue as SMs free up
     pdl_wait();               // everything before this kernel in the stream is complete and visible
+    //@T 2
 
     // ---- this CTA's work ----
     Work wk;
@@ -557,6 +583,8 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
         ti.row = ti.tree ? wk.b * pl.T_cap + ti.tt * kTileN : kv_row0 + j * kTileN;  // (contiguous KV)
         return ti;
     };
+    if (pair) asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+    //@T 3
     const uint16_t mc_mask = wk.share ? 3 : (uint16_t)(1u << (blockIdx.x & 1));
 
     // the control warpgroup hands registers to the two softmax warpgroups (one instruction per warpgroup)
@@ -627,6 +655,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
                     else tma_load_4d(dst, tm, fb, 0, ti.row, 0, wk.g, hint);
                 }
             }
+            //@T (jj < 6 ? 8 + jj : 63)
             if (is_v && (ti.valid & 15) != 0) {
                 mbar_wait(fb, (jj / ring) & 1);  // this fill has landed (every lane observes it)
                 const int n_rows = ((ti.valid + 15) & ~15) - ti.valid;
@@ -672,6 +701,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
                 }
                 tc_commit(bar(kBarSFull + s));
                 release(bar(kBarKEmpty + i));  // K_n is free once this Q.K^T has completed
+                //@T (n < 8 ? 16 + 2 * n : 63)
             };
             mbar_wait(bar(kBarQFull), 0);  // (also with N = 0: the CTA must not leave with the load in flight)
             if (N > 0) issue_qk(0);
@@ -702,6 +732,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
                 }
                 tc_commit(bar(kBarPFree + s));
                 release(bar(kBarVEmpty + vi));  // V_n is free once these P.V pieces have completed
+                //@T (n < 8 ? 17 + 2 * n : 63)
             }
             tc_commit(bar(kBarAllDone));
         }
@@ -731,6 +762,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
             const uint32_t sbuf = tmem + kTmemS + s * kTileN + lane_addr;
             const uint32_t pbuf = tmem + kTmemP + s * (kTileN / 2) + lane_addr;
             mbar_wait(bar(kBarSFull + s), par);
+            //@T (n < 8 ? 32 + 5 * (n >> 1) : 63)
             if (!warp_active) {  // a warp without rows only keeps the barrier phases in step
                 if (lane == 0) {
                     mbar_arrive(bar(kBarSFree + s));
@@ -750,6 +782,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(bar(kBarSFree + s));  // Q.K^T of unit n+2 may overwrite S now
+            //@T (n < 8 ? 33 + 5 * (n >> 1) : 63)
             if (ti.tree || ti.valid < kTileN) {
                 // keys past the tile's end, and (tree tiles) keys that are not ancestors-or-self of this
                 // row's node: the tile's 128 mask bits -> -inf
@@ -786,6 +819,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
                 xm[g * kTileM + rl] = m_new;
                 named_bar_arrive(1 + 4 * g + w, 64);
             }
+            //@T (n < 8 ? 34 + 5 * (n >> 1) : 63)
             if (m_new != m_mine) {  // this thread's own row sum follows the reference
                 l_mine *= m_mine == -INFINITY ? 0.f : ex2((m_mine - m_new) * c2);
                 m_mine = m_new;
@@ -825,6 +859,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
                     tc_fence_before();
                     __syncwarp();
                     if (lane == 0) mbar_arrive(bar(kBarPFull + 4 * s + q - 1));
+                    //@T (n < 8 && q == 1 ? 35 + 5 * (n >> 1) : 63)
                 }
                 uint32_t p[16];
                 float t0 = 0.f, t1 = 0.f, t2 = 0.f, t3 = 0.f;
@@ -843,6 +878,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(bar(kBarPFull + 4 * s + 3));
+            //@T (n < 8 ? 36 + 5 * (n >> 1) : 63)
         }
         // ---- epilogue: the two teams' row sums meet at the final reference; the normalised state leaves the
         // CTA straight from registers through a per-warp transpose in shared memory (the rings are free):
@@ -850,6 +886,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
         // runs.  A group with a single chunk writes its rows to `out` directly: no exchange at all. ----
         if (warp_active && N > 0 && ((N - 1) & 1) == g) xm[g * kTileM + rl] = m_mine;  // owner of the last unit
         mbar_wait(bar(kBarAllDone), 0);  // every MMA done: O is final, the rings are free
+        //@T 56
         named_bar_sync(9, 256);
         const float m_fin = N > 0 ? xm[((N - 1) & 1) * kTileM + rl] : -INFINITY;
         if (m_fin != m_mine) l_mine *= m_mine == -INFINITY ? 0.f : ex2((m_mine - m_fin) * c2);
@@ -859,47 +896,48 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
         const float l_tot = l_mine + xl[(g ^ 1) * kTileM + rl];
         const float inv = l_tot > 0.f ? 1.f / l_tot : 0.f;  // l = 0: every key of the chunk masked, or no key at all
         const float lse_v = l_tot > 0.f ? m_fin * pl.sm_scale + logf(l_tot) : -INFINITY;
+        //@T 57
         const bool direct = wk.n_chunks == 1;
         const bool row_ok = rl < wk.rows;
         const size_t prow0 = (size_t)wk.group * pl.grp_rows + (size_t)wk.chunk * kTileM;
         if (warp_active) {
-            const uint32_t region = smem + kOffK + (uint32_t)warp * 8192u;  // [32 rows][256 B], 16-byte chunks XOR-swizzled
-            tc_fence_after();
-#pragma unroll
-            for (int c0 = 0; c0 < 64; c0 += 32) {
-                uint32_t ov[32];
-                if (N > 0) {
-                    D2SD_TMEM_LD32(tmem + lane_addr + g * 64 + c0, ov, 0);
-                    tmem_wait_ld();
-                }
-#pragma unroll
-                for (int c = 0; c < 32; c += 4) {
-                    const uint32_t chunk = (uint32_t)((c0 + c) >> 2) ^ ((uint32_t)lane & 15u);
-                    float f0 = 0.f, f1 = 0.f, f2 = 0.f, f3 = 0.f;
-                    if (N > 0) {
-                        f0 = __uint_as_float(ov[c]) * inv; f1 = __uint_as_float(ov[c + 1]) * inv;
-                        f2 = __uint_as_float(ov[c + 2]) * inv; f3 = __uint_as_float(ov[c + 3]) * inv;
-                    }
-                    asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(region + (uint32_t)lane * 256u + chunk * 16u),
-                                 "f"(f0), "f"(f1), "f"(f2), "f"(f3)
-                                 : "memory");
-                }
-            }
-            __syncwarp();
+            // [32 rows][256 B] of fp32 (direct output) or [32 rows][128 B] of bf16 pairs (partial state), 16-byte
+            // chunks XOR-swizzled by the row
+            const uint32_t region = smem + kOffK + (uint32_t)warp * 8192u;
             const int G = pl.G;
+            tc_fence_after();
+            if (direct) {
+#pragma unroll
+                for (int c0 = 0; c0 < 64; c0 += 32) {
+                    uint32_t ov[32];
+                    if (N > 0) {
+                        D2SD_TMEM_LD32(tmem + lane_addr + g * 64 + c0, ov, 0);
+                        tmem_wait_ld();
+                    }
+#pragma unroll
+                    for (int c = 0; c < 32; c += 4) {
+                        const uint32_t chunk = (uint32_t)((c0 + c) >> 2) ^ ((uint32_t)lane & 15u);
+                        float f0 = 0.f, f1 = 0.f, f2 = 0.f, f3 = 0.f;
+                        if (N > 0) {
+                            f0 = __uint_as_float(ov[c]) * inv; f1 = __uint_as_float(ov[c + 1]) * inv;
+                            f2 = __uint_as_float(ov[c + 2]) * inv; f3 = __uint_as_float(ov[c + 3]) * inv;
+                        }
+                        asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(region + (uint32_t)lane * 256u + chunk * 16u),
+                                     "f"(f0), "f"(f1), "f"(f2), "f"(f3)
+                                     : "memory");
+                    }
+                }
+                __syncwarp();
 #pragma unroll 4
-            for (int it = 0; it < 16; ++it) {
-                const int row = it * 2 + (lane >> 4), ck = lane & 15;
-                float4 v;
-                asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];"
-                             : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
-                             : "r"(region + (uint32_t)row * 256u + (uint32_t)((ck ^ (row & 15)) * 16)));
-                const int r = w * 32 + row;  // row of the tile
-                if (r >= wk.rows) continue;
-                const int col = g * 64 + ck * 4;
-                if (!direct) {
-                    *reinterpret_cast<float4*>(a.part_o + (prow0 + r) * kD + col) = v;
-                } else {
+                for (int it = 0; it < 16; ++it) {
+                    const int row = it * 2 + (lane >> 4), ck = lane & 15;
+                    float4 v;
+                    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];"
+                                 : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
+                                 : "r"(region + (uint32_t)row * 256u + (uint32_t)((ck ^ (row & 15)) * 16)));
+                    const int r = w * 32 + row;  // row of the tile
+                    if (r >= wk.rows) continue;
+                    const int col = g * 64 + ck * 4;
                     const int ra = wk.row_base + r, t = ra / G;
                     const size_t orow = ((size_t)wk.b * pl.T_cap + t) * pl.Hq + wk.g * G + (ra - t * G);
                     if (dbg_rows) {
@@ -912,11 +950,45 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
                         *reinterpret_cast<uint2*>(a.out + orow * kD + col) = pk;
                     }
                 }
+            } else {
+#pragma unroll
+                for (int c0 = 0; c0 < 64; c0 += 32) {
+                    uint32_t ov[32];
+                    if (N > 0) {
+                        D2SD_TMEM_LD32(tmem + lane_addr + g * 64 + c0, ov, 0);
+                        tmem_wait_ld();
+                    }
+#pragma unroll
+                    for (int c = 0; c < 32; c += 8) {  // 8 columns = one 16-byte chunk of bf16
+                        const uint32_t chunk = (uint32_t)((c0 + c) >> 3) ^ ((uint32_t)lane & 7u);
+                        uint32_t pk[4] = {0u, 0u, 0u, 0u};
+                        if (N > 0) {
+#pragma unroll
+                            for (int e = 0; e < 4; ++e)
+                                pk[e] = pack2_bf16(__uint_as_float(ov[c + 2 * e]) * inv, __uint_as_float(ov[c + 2 * e + 1]) * inv);
+                        }
+                        asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(region + (uint32_t)lane * 128u + chunk * 16u),
+                                     "r"(pk[0]), "r"(pk[1]), "r"(pk[2]), "r"(pk[3])
+                                     : "memory");
+                    }
+                }
+                __syncwarp();
+#pragma unroll 4
+                for (int it = 0; it < 8; ++it) {
+                    const int row = it * 4 + (lane >> 3), ck = lane & 7;
+                    uint4 v;
+                    asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];"
+                                 : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w)
+                                 : "r"(region + (uint32_t)row * 128u + (uint32_t)((ck ^ (row & 7)) * 16)));
+                    const int r = w * 32 + row;  // row of the tile
+                    if (r < wk.rows) *reinterpret_cast<uint4*>(a.part_o16 + (prow0 + r) * kD + g * 64 + ck * 8) = v;
+                }
             }
             if (g == 0 && row_ok) {
                 if (!direct) {
                     a.part_lse[prow0 + rl] = lse_v;
                 } else {
+                    const int G = pl.G;
                     const int ra = wk.row_base + rl, t = ra / G;
                     const size_t orow = ((size_t)wk.b * pl.T_cap + t) * pl.Hq + wk.g * G + (ra - t * G);
                     if (dbg_rows) dbg_rows[orow * (kD + 1) + kD] = lse_v;
@@ -928,15 +1000,18 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
             // ---- publish this CTA's partial state, wait for the group, merge this CTA's share of rows ----
             const unsigned expected = (unsigned)wk.n_chunks;
             unsigned* cnt = a.counters + 2 * wk.group;  // [0] arrivals, [1] done
-            __threadfence();
-            named_bar_sync(9, 256);  // every thread's partial-state writes happen before the leader's release
+            named_bar_sync(9, 256);  // every thread's partial-state writes happen before the leader's (cumulative) release
+            //@T 58
             unsigned done_before = 0;
             int ok = 1;
             if (warp == 0 && lane == 0) {
+                __threadfence();
                 asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(cnt) : "memory");
                 unsigned seen, spins = 0;
                 do {
-                    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(cnt) : "memory");
+                    // relaxed: the states are read with L2-level loads (ld.global.cg) issued after this load has
+                    // returned; an acquire here would invalidate the whole L1 on every poll
+                    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(cnt) : "memory");
                     if (seen < expected) {
                         __nanosleep(20);
                         if (++spins > (1u << 22)) {  // the group never became co-resident: report, do not hang
@@ -951,8 +1026,10 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
                 xl[0] = __int_as_float(ok);
             }
             named_bar_sync(10, 256);
+            //@T 59
             if (__float_as_int(xl[0]))
-                merge_rows(pl, a, dbg_rows, wk, reinterpret_cast<float*>(smem_gen + kOffV), warp, lane);
+                merge_rows(pl, a, dbg_rows, wk, warp, lane);
+            //@T 60
             if (warp == 0 && lane == 0) {
                 if (done_before == expected - 1) {  // last CTA out: everybody is past the wait
                     cnt[0] = 0;
@@ -968,7 +1045,9 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
     if (warp == 10) {
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(kTmemCols) : "memory");
     }
+    //@T 61
     if (pair) cluster_sync_all();  // no CTA leaves while its peer may still signal its barriers
+    //@T 62
 }
 
 // ---- host side ----------------------------------------------------------------------------------

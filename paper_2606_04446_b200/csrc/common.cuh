@@ -139,6 +139,7 @@ struct AttnArgs {
     __nv_bfloat16* out;
     float *lse, *dbg_state;
     float *part_o, *part_lse;
+    __nv_bfloat16* part_o16;  // one-tile-per-CTA kernel: partial O rows in bf16
     unsigned* counters;  // tcgen05 path only: [group][2] arrivals / done
 };
 
