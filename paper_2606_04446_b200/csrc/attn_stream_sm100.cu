@@ -13,28 +13,31 @@
 // multicast into both CTAs' rings, so a KV tile crosses the L2->SM fabric once per 256 query rows --
 // and the chunks of an odd last M tile are paired without sharing.
 //
-// TMEM (512 columns): O (128 fp32 columns), S_0, S_1 (128 each), P_0, P_1 (64 each, bf16 pairs).
-// Unit n uses buffers n & 1.  S and P are separate columns, so Q.K^T of unit n+2 is issued as soon as
-// the softmax has READ S_n (it does not wait for P.V of unit n), and the softmax never waits for the
-// tensor pipe in steady state:
+// TMEM (512 columns): O (128 fp32 columns), S_0..S_3 (64 each), P_0..P_3 (32 each, bf16 pairs).
+// A 128-key tile is processed as two 64-key SUB-UNITS; sub-unit n uses buffers n & 3.  S and P are
+// separate columns, so Q.K^T of sub-unit n+4 is issued as soon as the softmax has READ S_n (it does not
+// wait for P.V of sub-unit n), and the softmax never waits for the tensor pipe in steady state:
 //
-//   S_n[128 x 128] = Q[128 x 128] . K_n^T        tcgen05.mma, A/B from 128B-swizzled SMEM (TMA)
-//   P_n            = exp2(c*(S_n - m_ref))       one softmax thread per row (TMEM lane)
-//   O[128 x 128]  += P_n[128 x 128] . V_n        tcgen05.mma, A = P from TMEM, B = V (MN-major SMEM)
+//   S_n[128 x 64] = Q[128 x 128] . K_n^T         tcgen05.mma, A/B from 128B-swizzled SMEM (TMA)
+//   P_n           = exp2(c*(S_n - m_ref))        one softmax thread per row (TMEM lane)
+//   O[128 x 128] += P_n[128 x 64] . V_n          tcgen05.mma, A = P from TMEM, B = V (MN-major SMEM)
 //
-// Warp roles (384 threads): warps 0..3 = softmax team A (even units), warps 4..7 = team B (odd units),
-// thread (w, lane) of either team owns query row w*32 + lane; warp 8 = K producer (+ Q), warp 9 =
-// V producer (also zeroes the V rows behind a ragged tile end: they are multiplied by exact zeros
-// and may hold anything, NaN included), warp 10 = MMA issuer (one elected thread; owns the TMEM
-// allocation), warp 11 idle.  The two teams work on different units at the same time, so one team's
-// loads / maxima / packs overlap the other's exponentials on the shared MUFU pipe.
+// Warp roles (640 threads): warps 0..15 = four softmax teams of four warps, team t owns the sub-units
+// n = t (mod 4), thread (w, lane) of a team owns query row w*32 + lane (TMEM lane) and the 64 scores of
+// the sub-unit; warp 16 = K producer (+ Q), warp 17 = V producer (also zeroes the V rows behind a
+// ragged tile end: they are multiplied by exact zeros and may hold anything, NaN included), warp 18 =
+// Q.K^T issuer (one elected thread; owns the TMEM allocation), warp 19 = P.V issuer.  A single softmax warp runs
+// at ~0.2 instructions per clock (dependent chains of the maxima, exponentials, packs): four teams keep
+// four warps per scheduler busy on four different sub-units, so one team's loads / maxima / packs
+// overlap the others' exponentials on the shared MUFU pipe, inside the register file's 64 Ki registers
+// (64 scores per thread: 112 registers).
 //
-// One accumulator, two teams: the row's reference maximum m_ref travels with the unit sequence.  The
-// owner of unit n reads m_ref(n-1) from shared memory (published by the other team, ordered by a
-// 64-thread named barrier per warp pair), raises it only when the tile maximum exceeds it by more than
-// 2^8 (lazy rescale), publishes m_ref(n), and -- only when it raised it -- waits for P.V of unit n-1
-// and rescales its O row in TMEM before it releases P_n.  Each thread keeps its own row sum relative
-// to the last reference it has seen; the two sums meet in the epilogue.
+// One accumulator, four teams: the row's reference maximum m_ref travels with the sub-unit sequence.
+// The owner of sub-unit n reads m_ref(n-1) from shared memory (published by the previous team's warp of
+// the same rows, ordered by an mbarrier per (team, warp)), raises it only when the tile maximum exceeds
+// it by more than 2^8 (lazy rescale), publishes m_ref(n), and -- only when it raised it -- waits for
+// P.V of sub-unit n-1 and rescales its O row in TMEM before it releases P_n.  Each thread keeps its own
+// row sum relative to the last reference it has seen; the four sums meet in the epilogue.
 //
 // Cascade merge in the same launch (log-sum-exp state merge): every CTA writes its
 // normalised partial state (O fp32, LSE) to the workspace straight from registers (tcgen05.ld 16x256b
@@ -59,23 +62,25 @@ constexpr int kD = 128;
 constexpr int kTileM = 128;
 constexpr int kTileN = 128;
 constexpr int kRingK = 3, kRingV = 3;  // K tiles / V tiles in flight or in use
-constexpr int kThreads = 384;
+constexpr int kThreads = 640;      // 16 softmax warps (4 teams) + 4 control warps
+constexpr int kTeams = 4;
+constexpr int kSubN = 64;          // keys per sub-unit (one S / P buffer)
 constexpr uint32_t kQTileBytes = kTileM * kD * 2;   // 32 KiB: [d_hi 2][128 rows][128 B]
 constexpr uint32_t kKvTileBytes = kTileN * kD * 2;  // 32 KiB: [d_hi 2][128 keys][128 B]
 constexpr uint32_t kOffQ = 0;
 constexpr uint32_t kOffK = kQTileBytes;
 constexpr uint32_t kOffV = kOffK + kRingK * kKvTileBytes;
 constexpr uint32_t kOffBar = kOffV + kRingV * kKvTileBytes;
-constexpr uint32_t kOffX = kOffBar + 256;                 // reference-maximum hand-off: fp32 [2 teams][128 rows]
-constexpr uint32_t kOffXL = kOffX + 2 * kTileM * 4;         // row sums of the two teams: fp32 [2][128]
-constexpr uint32_t kSmemUsed = kOffXL + 2 * kTileM * 4;
+constexpr uint32_t kOffX = kOffBar + 512;                 // reference-maximum hand-off: fp32 [4 teams][128 rows]
+constexpr uint32_t kOffXL = kOffX;                        // epilogue: the teams' row sums take the same place
+constexpr uint32_t kSmemUsed = kOffX + kTeams * kTileM * 4;
 constexpr uint32_t kSmemBytes = 232448;                   // the whole 227 KiB: kSmemUsed + alignment slack
 constexpr uint32_t kTmemCols = 512;
-constexpr uint32_t kTmemS = 128;   // S_0, S_1 behind O
-constexpr uint32_t kTmemP = 384;   // P_0, P_1 (64 columns each)
+constexpr uint32_t kTmemS = 128;   // S_0..S_3 behind O (64 fp32 columns each)
+constexpr uint32_t kTmemP = 384;   // P_0..P_3 (32 columns of bf16 pairs each)
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kRescaleThreshold = 8.0f;  // log2 units
-constexpr uint32_t kRegsControl = 80, kRegsSoftmax = 208;  // setmaxnreg targets
+constexpr uint32_t kRegsControl = 64, kRegsSoftmax = 104;  // setmaxnreg targets: 512 x 104 + 128 x 64 = 60 Ki registers (the launch allocation)
 
 // barrier slots (8 bytes each) at kOffBar
 enum : uint32_t {
@@ -84,17 +89,18 @@ enum : uint32_t {
     kBarKEmpty = kBarKFull + kRingK,     // [kRingK]
     kBarVFull = kBarKEmpty + kRingK,     // [kRingV]
     kBarVEmpty = kBarVFull + kRingV,     // [kRingV]
-    kBarSFull = kBarVEmpty + kRingV,     // [2] Q.K^T of a unit has completed
-    kBarSFree = kBarSFull + 2,           // [2] the owning team has read S into registers
-    kBarPFull = kBarSFree + 2,           // [2][4] P is released to the tensor pipe in four 32-key pieces
-    kBarPFree = kBarPFull + 8,           // [2] P.V of a unit has completed (P buffer reusable, O current)
-    kBarVFix = kBarPFree + 2,            // [2] V rows behind a ragged tile end are zero (<= 2 ragged tiles per CTA)
+    kBarSFull = kBarVEmpty + kRingV,     // [4] Q.K^T of a sub-unit has completed
+    kBarSFree = kBarSFull + kTeams,      // [4] the owning team has read S into registers
+    kBarPFull = kBarSFree + kTeams,      // [4] the owning team has written P
+    kBarPFree = kBarPFull + kTeams,      // [4] P.V of a sub-unit has completed (P buffer reusable, O current)
+    kBarRef = kBarPFree + kTeams,        // [4 teams][4 warps] the team's warp has published its rows' reference maxima
+    kBarVFix = kBarRef + 4 * kTeams,     // [2] V rows behind a ragged tile end are zero (<= 2 ragged tiles per CTA)
     kBarAllDone = kBarVFix + 2,
     kNumBars = kBarAllDone + 1,
     kTmemSlot = kNumBars  // uint32 written by tcgen05.alloc
 };
-static_assert((kNumBars + 1) * 8 <= 256, "barrier area");
-static_assert(kSmemUsed + 768 <= kSmemBytes, "shared memory budget");  // the kernel checks the actual alignment slack
+static_assert((kNumBars + 1) * 8 <= 512, "barrier area");
+static_assert(kSmemUsed + 512 <= kSmemBytes, "shared memory budget");  // the kernel checks the actual alignment slack
 
 // ---- PTX wrappers -------------------------------------------------------------------------------
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
@@ -360,7 +366,7 @@ struct TileInfo {
 
 __device__ __forceinline__ uint2 ld_cg_u2(const __nv_bfloat16* p) {
     uint2 v;
-    asm volatile("ld.global.cg.v2.u32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "l"(p));
+    asm volatile("ld.global.v2.u32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "l"(p));
     return v;
 }
 __device__ __forceinline__ float bf_lo(uint32_t w) { return __uint_as_float(w << 16); }
@@ -370,9 +376,9 @@ __device__ __forceinline__ float bf_hi(uint32_t w) { return __uint_as_float(w & 
 // Cascade merge of one group's rows (log-sum-exp state merge):
 //   LSE = log sum_p e^{LSE_p};  O = sum_p e^{LSE_p - LSE} O_p   over the group's chunk states.
 // CTA `chunk` of the group's n_chunks CTAs takes a contiguous range of the tile's rows; a warp takes
-// three rows at a time.  Everything a warp needs for its rows is requested at once -- lane i loads the
+// two rows at a time.  Everything a warp needs for its rows is requested at once -- lane i loads the
 // LSE of state i, every lane loads its 16-byte piece of every state's O row (512 contiguous bytes per
-// warp instruction, up to eight states x three rows in flight) -- so the merge costs one L2 round trip;
+// warp instruction, up to eight states x two rows in flight) -- so the merge costs one L2 round trip;
 // the weights are reduced with shuffles and never leave the registers.  The partial states were written
 // by other SMs and published with a release; they are read at L2 (ld.global.cg).
 __device__ __forceinline__ void merge_rows(const AttnPlan& pl, const AttnArgs& a, float* dbg_rows, const Work& wk,
@@ -382,16 +388,16 @@ __device__ __forceinline__ void merge_rows(const AttnPlan& pl, const AttnArgs& a
     const size_t grp0 = (size_t)wk.group * pl.grp_rows;
     const int r0 = wk.rows * wk.chunk / nc, r1 = wk.rows * (wk.chunk + 1) / nc;
     const int nrows = r1 - r0;  // <= 128
-    constexpr int kRB = 3, kSB = 8;
-    for (int rb = warp * kRB; rb < nrows; rb += 8 * kRB) {
-        // lane i holds LSE of states i and i + 32 for each of the three rows
+    constexpr int kRB = 2, kSB = 8;
+    for (int rb = warp * kRB; rb < nrows; rb += 16 * kRB) {
+        // lane i holds LSE of states i and i + 32 for each of the two rows
         float lv[kRB][2];
 #pragma unroll
         for (int u = 0; u < kRB; ++u)
 #pragma unroll
             for (int hh = 0; hh < 2; ++hh) {
                 const int i = lane + 32 * hh;
-                lv[u][hh] = (rb + u < nrows && i < nc) ? __ldcg(a.part_lse + grp0 + (size_t)i * kTileM + r0 + rb + u) : -INFINITY;
+                lv[u][hh] = (rb + u < nrows && i < nc) ? a.part_lse[grp0 + (size_t)i * kTileM + r0 + rb + u] : -INFINITY;
             }
         uint2 v[kRB][kSB];
 #pragma unroll
@@ -494,7 +500,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
     const bool pair = (int)blockIdx.x < pair_ctas;  // cluster of M tiles (2p, 2p+1) over one chunk
 
     // ---- prologue that touches no global memory (overlaps the preceding kernel's tail under PDL) ----
-    if (warp == 8 && lane == 0) {
+    if (warp == 16 && lane == 0) {
         mbar_init(bar(kBarQFull), 1);
         for (int i = 0; i < kRingK; ++i) {
             mbar_init(bar(kBarKFull + i), 1);
@@ -504,13 +510,15 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
             mbar_init(bar(kBarVFull + i), 1);
             mbar_init(bar(kBarVEmpty + i), pair ? 2 : 1);
         }
-        for (int s = 0; s < 2; ++s) {
-            mbar_init(bar(kBarSFull + s), 1);
-            mbar_init(bar(kBarSFree + s), 4);  // one elected arrival per warp of the owning team
-            for (int q = 0; q < 4; ++q) mbar_init(bar(kBarPFull + 4 * s + q), 4);
-            mbar_init(bar(kBarPFree + s), 1);
-            mbar_init(bar(kBarVFix + s), 1);
+        for (int t = 0; t < kTeams; ++t) {
+            mbar_init(bar(kBarSFull + t), 1);
+            mbar_init(bar(kBarSFree + t), 4);  // one elected arrival per warp of the owning team
+            mbar_init(bar(kBarPFull + t), 4);
+            mbar_init(bar(kBarPFree + t), 1);
+            for (int w = 0; w < 4; ++w) mbar_init(bar(kBarRef + 4 * t + w), 1);
         }
+        mbar_init(bar(kBarVFix + 0), 1);
+        mbar_init(bar(kBarVFix + 1), 1);
         mbar_init(bar(kBarAllDone), 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         tma_prefetch_desc(&tm_q);
@@ -519,7 +527,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
         tma_prefetch_desc(&tm_tk);
         tma_prefetch_desc(&tm_tv);
     }
-    if (warp == 10) {
+    if (warp == 18) {
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(bar(kTmemSlot)),
                      "r"(kTmemCols)
                      : "memory");
@@ -588,11 +596,11 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
     const uint16_t mc_mask = wk.share ? 3 : (uint16_t)(1u << (blockIdx.x & 1));
 
     // the control warpgroup hands registers to the two softmax warpgroups (one instruction per warpgroup)
-    if (warp >= 8) {
+    if (warp >= 16) {
       asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsControl));
       if (idle) {
         // fall through to the TMEM release
-      } else if (warp == 8 || warp == 9) {
+      } else if (warp == 16 || warp == 17) {
         // ===== K producer (warp 8, also loads Q) and V producer (warp 9): one ring of three tiles each.
         // Contiguous KV: lane 0 issues one 32 KiB box per tile.  Paged KV (page = 16 keys): a 128-key
         // tile is 8 pages; lane 2p+hi issues the 2 KiB box (page p, d half hi), so a tile is 16 loads in
@@ -604,7 +612,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
         // runs over ceil16(valid) keys, rows valid..ceil16(valid)-1 belong to nobody (next request, tree
         // padding), are multiplied by P = 0 exactly and must not hold NaN/Inf.  A row is 2 x 128 B (d
         // halves); the 128B swizzle permutes 16-byte chunks inside a row's 128 B only. =====
-        const bool is_v = warp == 9;
+        const bool is_v = warp == 17;
         const bool paged = pl.page_size > 0;
         const bool issuer = !wk.share || wk.rank == (is_v ? 1 : 0);
         const int ring = is_v ? kRingV : kRingK;
@@ -673,11 +681,12 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
             __syncwarp();
             page_cur = page_next;
         }
-      } else if (warp == 10) {
-        // ===== MMA issuer: one elected thread walks the unit sequence.  Q.K^T of unit n+2 goes out as soon
-        // as the owning team has read S_n (S and P are separate TMEM columns), P.V of unit n as its P pieces
-        // arrive; the tensor pipe executes them in this order.  A ring slot is released by the commit behind
-        // its last reader (to both CTAs of a sharing pair). =====
+      } else if (warp == 18 || warp == 19) {
+        // ===== MMA issuers (warp 18: Q.K^T stream, warp 19: P.V stream): one elected thread each walks the sub-unit sequence (two 64-key halves per key tile, a
+        // ragged tile's second half only if it holds keys).  Q.K^T of sub-unit n+4 goes out as soon as the
+        // owning team has read S_n (S and P are separate TMEM columns), P.V of sub-unit n as its P arrives;
+        // the tensor pipe executes them in this order.  A ring slot is released by the commit behind its
+        // last reader (to both CTAs of a sharing pair). =====
         if (elect_one()) {
             const uint64_t qd = smem_desc(smem + kOffQ, 16, 1024);
             const uint32_t od = tmem;
@@ -686,214 +695,243 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
                 if (wk.share) tc_commit_mc(b, 3);
                 else { tc_commit(b); if (pair) tc_commit(b); }  // a pair cluster's barriers count two releases
             };
-            auto issue_qk = [&](int n) {
-                const int i = n % kRingK, s = n & 1;
-                mbar_wait(bar(kBarKFull + i), (n / kRingK) & 1);
-                const int tile_n = (tile_info(n).valid + 15) & ~15;  // MMA N (multiple of 16)
-                const uint64_t kd = smem_desc(smem + kOffK + i * kKvTileBytes, 16, 1024);
-                const uint32_t id_qk = idesc(kTileM, (uint32_t)tile_n, 0);
-                const uint32_t sd = tmem + kTmemS + s * kTileN;
+            // cursor over the sub-unit sequence: key tile jj, half hf, keys of the half
+            struct Cur { int n, jj, hf, valid; };
+            auto cur_keys = [&](const Cur& c) { return min(kSubN, c.valid - c.hf * kSubN); };
+            auto cur_last_half = [&](const Cur& c) { return (c.hf + 1) * kSubN >= c.valid; };
+            auto cur_next = [&](Cur& c) {
+                ++c.n;
+                if (cur_last_half(c)) { ++c.jj; c.hf = 0; c.valid = c.jj < N ? tile_info(c.jj).valid : 0; }
+                else ++c.hf;
+            };
+            auto issue_qk = [&](const Cur& c) {
+                const int i = c.jj % kRingK, t = c.n & 3;
+                if (c.hf == 0) mbar_wait(bar(kBarKFull + i), (c.jj / kRingK) & 1);
+                const int n_cols = (cur_keys(c) + 15) & ~15;  // MMA N (multiple of 16)
+                const uint64_t kd = smem_desc(smem + kOffK + i * kKvTileBytes + (uint32_t)c.hf * (kSubN * 128u), 16, 1024);
+                const uint32_t id_qk = idesc(kTileM, (uint32_t)n_cols, 0);
+                const uint32_t sd = tmem + kTmemS + t * kSubN;
                 tc_fence_after();
 #pragma unroll
                 for (int kk = 0; kk < kD / 16; ++kk) {
                     const uint64_t off = (uint64_t)(((kk >> 2) * (kQTileBytes / 2) + (kk & 3) * 32) >> 4);
                     umma_ss(sd, qd + off, kd + off, id_qk, kk > 0);
                 }
-                tc_commit(bar(kBarSFull + s));
-                release(bar(kBarKEmpty + i));  // K_n is free once this Q.K^T has completed
-                //@T (n < 8 ? 16 + 2 * n : 63)
+                tc_commit(bar(kBarSFull + t));
+                if (cur_last_half(c)) release(bar(kBarKEmpty + i));  // K is free once the tile's last Q.K^T has completed
+                //@T (c.n < 8 ? 16 + 2 * c.n : 63)
             };
-            mbar_wait(bar(kBarQFull), 0);  // (also with N = 0: the CTA must not leave with the load in flight)
-            if (N > 0) issue_qk(0);
-            if (N > 1) issue_qk(1);
-            uint32_t n_ragged = 0;
-            for (int n = 0; n < N; ++n) {
-                const int s = n & 1, par = (n >> 1) & 1;
-                if (n + 2 < N) {
-                    mbar_wait(bar(kBarSFree + s), par);  // S_n is in the team's registers
-                    issue_qk(n + 2);
+            if (warp == 18) {
+                // Q.K^T stream: sub-unit n goes out as soon as its S buffer has been read (sub-unit n-4) and its K
+                // tile has landed
+                mbar_wait(bar(kBarQFull), 0);  // (also with N = 0: the CTA must not leave with the load in flight)
+                Cur qc{0, 0, 0, N > 0 ? tile_info(0).valid : 0};
+                while (qc.jj < N) {
+                    if (qc.n >= kTeams) mbar_wait(bar(kBarSFree + (qc.n & 3)), ((qc.n >> 2) & 1) ^ 1);
+                    issue_qk(qc);
+                    cur_next(qc);
                 }
-                const int valid = tile_info(n).valid;
-                const int ksteps = ((valid + 15) & ~15) >> 4;  // K extent of P.V in 16-key steps
-                const int vi = n % kRingV;
-                mbar_wait(bar(kBarVFull + vi), (n / kRingV) & 1);
-                if (valid & 15) mbar_wait(bar(kBarVFix + n_ragged++), 0);
-                const uint64_t vd = smem_desc(smem + kOffV + vi * kKvTileBytes, kKvTileBytes / 2, 1024);
-                const uint32_t pd = tmem + kTmemP + s * (kTileN / 2);
-#pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    // every piece is awaited, also the ones past a ragged tile's end that feed no MMA (the
-                    // barrier phases stay in step)
-                    mbar_wait(bar(kBarPFull + 4 * s + q), par);
+            } else {
+                // P.V stream: sub-unit n goes out as its P arrives; the last commit covers every P.V, and every
+                // Q.K^T has completed before its scores were read
+                Cur pc{0, 0, 0, N > 0 ? tile_info(0).valid : 0};
+                uint32_t n_ragged = 0;
+                while (pc.jj < N) {
+                    const int t = pc.n & 3, par = (pc.n >> 2) & 1;
+                    const int vi = pc.jj % kRingV;
+                    if (pc.hf == 0) {
+                        mbar_wait(bar(kBarVFull + vi), (pc.jj / kRingV) & 1);
+                        if (pc.valid & 15) mbar_wait(bar(kBarVFix + n_ragged++), 0);
+                    }
+                    const int ksteps = ((cur_keys(pc) + 15) & ~15) >> 4;  // K extent of this P.V in 16-key steps
+                    const uint64_t vd = smem_desc(smem + kOffV + vi * kKvTileBytes, kKvTileBytes / 2, 1024);
+                    const uint32_t pd = tmem + kTmemP + t * (kSubN / 2);
+                    mbar_wait(bar(kBarPFull + t), par);
                     tc_fence_after();
 #pragma unroll
-                    for (int ks = 2 * q; ks < 2 * q + 2; ++ks)
-                        if (ks < ksteps) umma_ts(od, pd + ks * 8, vd + (uint64_t)(ks * (2048 >> 4)), kIdescPV, (n > 0) | ks);
+                    for (int ks = 0; ks < kSubN / 16; ++ks)
+                        if (ks < ksteps)
+                            umma_ts(od, pd + ks * 8, vd + (uint64_t)((pc.hf * (kSubN / 16) + ks) * (2048 >> 4)), kIdescPV, (pc.n > 0) | ks);
+                    tc_commit(bar(kBarPFree + t));
+                    if (cur_last_half(pc)) release(bar(kBarVEmpty + vi));  // V is free once the tile's last P.V has completed
+                    //@T (pc.n < 8 ? 17 + 2 * pc.n : 63)
+                    cur_next(pc);
                 }
-                tc_commit(bar(kBarPFree + s));
-                release(bar(kBarVEmpty + vi));  // V_n is free once these P.V pieces have completed
-                //@T (n < 8 ? 17 + 2 * n : 63)
+                tc_commit(bar(kBarAllDone));
             }
-            tc_commit(bar(kBarAllDone));
         }
       }
     } else {
       asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegsSoftmax));
       if (!idle) {
-        // ===== softmax: team A (warps 0..3) owns the even units, team B (warps 4..7) the odd ones; thread
-        // (w, lane) of either team owns query row w*32 + lane (TMEM lane) and a whole 128-key score row.
-        // While one team is in its exponentials the other loads, takes maxima, packs and stores. =====
-        const int g = warp >> 2;       // team
+        // ===== softmax: team t (warps 4t..4t+3) owns the sub-units n = t (mod 4); thread (w, lane) owns query
+        // row w*32 + lane (TMEM lane) and the sub-unit's 64 scores.  Four warps per scheduler work on four
+        // different sub-units: while one is in its exponentials the others load, take maxima, pack, store. =====
+        const int t = warp >> 2;       // team
         const int w = warp & 3;
         const int rl = w * 32 + lane;  // row within the tile
         const uint32_t lane_addr = (uint32_t)(w * 32) << 16;
         const float c2 = pl.sm_scale * kLog2e;
         const float thr = kRescaleThreshold / c2;  // in raw score units
-        float* xm = reinterpret_cast<float*>(smem_gen + kOffX);  // [team][row]: reference maximum after the team's last unit
+        float* xm = reinterpret_cast<float*>(smem_gen + kOffX);  // [team][row]: reference maximum after the team's last sub-unit
         const bool warp_active = w * 32 < wk.rows;
         const int N = wk.n_tiles;
         float m_mine = -INFINITY;  // the reference this thread's row sum is relative to
         float l_mine = 0.f;
         const int t_node = min((wk.row_base + rl) / pl.G, wk.T - 1);
         const uint32_t* mrow = a.mask + ((size_t)wk.b * pl.T_cap + t_node) * pl.W;
-        for (int n = g; n < N; n += 2) {
-            const int s = g, par = (n >> 1) & 1;
-            const TileInfo ti = tile_info(n);
-            const uint32_t sbuf = tmem + kTmemS + s * kTileN + lane_addr;
-            const uint32_t pbuf = tmem + kTmemP + s * (kTileN / 2) + lane_addr;
-            mbar_wait(bar(kBarSFull + s), par);
-            //@T (n < 8 ? 32 + 5 * (n >> 1) : 63)
-            if (!warp_active) {  // a warp without rows only keeps the barrier phases in step
-                if (lane == 0) {
-                    mbar_arrive(bar(kBarSFree + s));
-                    if (n >= 2) mbar_wait(bar(kBarPFree + s), par ^ 1);
-                    for (int q = 0; q < 4; ++q) mbar_arrive(bar(kBarPFull + 4 * s + q));
+        const uint32_t sbuf = tmem + kTmemS + t * kSubN + lane_addr;
+        const uint32_t pbuf = tmem + kTmemP + t * (kSubN / 2) + lane_addr;
+        const int tp = (t + kTeams - 1) & 3;  // the team that owns sub-unit n-1
+        int n = 0, n_sub = 0;                 // n: running sub-unit index; n_sub: total, known after the walk
+        for (int jj = 0; jj < N; ++jj) {
+            const TileInfo ti = tile_info(jj);
+            const int halves = (ti.valid + kSubN - 1) / kSubN;
+            for (int hf = 0; hf < halves; ++hf, ++n) {
+                if ((n & 3) != t) continue;
+                const int par = (n >> 2) & 1;
+                const int keys = min(kSubN, ti.valid - hf * kSubN);
+                const bool last = jj == N - 1 && hf == halves - 1;
+                mbar_wait(bar(kBarSFull + t), par);
+                //@T (n < 12 ? 32 + (n >> 2) * 5 : 63)
+                if (!warp_active) {  // a warp without rows only keeps the barrier phases in step
+                    if (lane == 0) {
+                        mbar_arrive(bar(kBarSFree + t));
+                        if (n >= kTeams) mbar_wait(bar(kBarPFree + t), par ^ 1);
+                        mbar_arrive(bar(kBarPFull + t));
+                    }
+                    __syncwarp();
+                    continue;
                 }
-                __syncwarp();
-                continue;
-            }
-            uint32_t sv[128];
-            tc_fence_after();
-            D2SD_TMEM_LD32(sbuf, sv, 0);
-            D2SD_TMEM_LD32(sbuf + 32, sv, 32);
-            D2SD_TMEM_LD32(sbuf + 64, sv, 64);
-            D2SD_TMEM_LD32(sbuf + 96, sv, 96);
-            tmem_wait_ld();
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(bar(kBarSFree + s));  // Q.K^T of unit n+2 may overwrite S now
-            //@T (n < 8 ? 33 + 5 * (n >> 1) : 63)
-            if (ti.tree || ti.valid < kTileN) {
-                // keys past the tile's end, and (tree tiles) keys that are not ancestors-or-self of this
-                // row's node: the tile's 128 mask bits -> -inf
-                uint32_t mw[4] = {0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu};
-                if (ti.tree) {
-#pragma unroll
-                    for (int u = 0; u < 4; ++u) mw[u] = ti.tt * 4 + u < pl.W ? mrow[ti.tt * 4 + u] : 0u;
-                }
-#pragma unroll
-                for (int c = 0; c < 128; ++c) {
-                    const uint32_t bit = (mw[c >> 5] >> (c & 31)) & 1u;
-                    if (c >= ti.valid || !bit) sv[c] = 0xFF800000u;
-                }
-            }
-            float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;
-#pragma unroll
-            for (int c = 0; c < 128; c += 4) {
-                mx0 = fmaxf(mx0, __uint_as_float(sv[c]));
-                mx1 = fmaxf(mx1, __uint_as_float(sv[c + 1]));
-                mx2 = fmaxf(mx2, __uint_as_float(sv[c + 2]));
-                mx3 = fmaxf(mx3, __uint_as_float(sv[c + 3]));
-            }
-            const float mx = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
-            // reference hand-off: m_ref(n-1) from the other team (ordered by the warp pair's named barrier),
-            // lazy raise, m_ref(n) to the other team
-            float m_prev = -INFINITY;
-            if (n > 0) {
-                named_bar_sync(1 + 4 * (g ^ 1) + w, 64);
-                m_prev = xm[(g ^ 1) * kTileM + rl];
-            }
-            const bool need = n > 0 && mx > m_prev + thr;
-            const float m_new = n == 0 ? mx : (need ? mx : m_prev);
-            if (n + 1 < N) {
-                xm[g * kTileM + rl] = m_new;
-                named_bar_arrive(1 + 4 * g + w, 64);
-            }
-            //@T (n < 8 ? 34 + 5 * (n >> 1) : 63)
-            if (m_new != m_mine) {  // this thread's own row sum follows the reference
-                l_mine *= m_mine == -INFINITY ? 0.f : ex2((m_mine - m_new) * c2);
-                m_mine = m_new;
-            }
-            if (__any_sync(0xffffffffu, need)) {
-                // O holds units < n relative to m_prev: wait for P.V of unit n-1 (the other buffer's), rescale
-                // this row.  P.V of unit n cannot start before this thread releases P_n below.
-                mbar_wait(bar(kBarPFree + (s ^ 1)), ((n - 1) >> 1) & 1);
+                uint32_t sv[kSubN];
                 tc_fence_after();
-                const float alpha = need ? (m_prev == -INFINITY ? 0.f : ex2((m_prev - m_new) * c2)) : 1.f;
-#pragma unroll 1
-                for (int c0 = 0; c0 < kD; c0 += 32) {
-                    uint32_t o[32];
-                    D2SD_TMEM_LD32(tmem + lane_addr + c0, o, 0);
-                    tmem_wait_ld();
-#pragma unroll
-                    for (int c = 0; c < 32; ++c) o[c] = __float_as_uint(__uint_as_float(o[c]) * alpha);
-                    D2SD_TMEM_ST32(tmem + lane_addr + c0, o, 0);
-                }
-                tmem_wait_st();
+                D2SD_TMEM_LD32(sbuf, sv, 0);
+                D2SD_TMEM_LD32(sbuf + 32, sv, 32);
+                tmem_wait_ld();
                 tc_fence_before();
-            }
-            // the P buffer is free once P.V of unit n-2 has completed
-            if (n >= 2) mbar_wait(bar(kBarPFree + s), par ^ 1);
-            // a row with every key so far masked has m_ref = -inf: exp2(-inf - 0) = 0, not NaN
-            const float ms = m_new == -INFINITY ? 0.f : m_new * c2;
-            float sum0 = 0.f, sum1 = 0.f;
-            // P[128 x 128] bf16 = 64 TMEM columns, written and released in four 32-key pieces; the store of a
-            // piece is only waited for after the next piece's exponentials
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar(kBarSFree + t));  // Q.K^T of sub-unit n+4 may overwrite S now
+                //@T (n < 12 ? 33 + (n >> 2) * 5 : 63)
+                if (ti.tree || keys < kSubN) {
+                    // keys past the tile's end, and (tree tiles) keys that are not ancestors-or-self of this
+                    // row's node: the sub-unit's 64 mask bits -> -inf
+                    uint32_t mw0 = 0xFFFFFFFFu, mw1 = 0xFFFFFFFFu;
+                    if (ti.tree) {
+                        const int wi = ti.tt * 4 + hf * 2;
+                        mw0 = wi < pl.W ? mrow[wi] : 0u;
+                        mw1 = wi + 1 < pl.W ? mrow[wi + 1] : 0u;
+                    }
 #pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                float ev[32];
+                    for (int c = 0; c < kSubN; ++c) {
+                        const uint32_t bit = ((c < 32 ? mw0 : mw1) >> (c & 31)) & 1u;
+                        if (c >= keys || !bit) sv[c] = 0xFF800000u;
+                    }
+                }
+                float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;
 #pragma unroll
-                for (int c = 0; c < 32; ++c) ev[c] = ex2_ordered(__uint_as_float(sv[q * 32 + c]) * c2 - ms);
-                if (q > 0) {
+                for (int c = 0; c < kSubN; c += 4) {
+                    mx0 = fmaxf(mx0, __uint_as_float(sv[c]));
+                    mx1 = fmaxf(mx1, __uint_as_float(sv[c + 1]));
+                    mx2 = fmaxf(mx2, __uint_as_float(sv[c + 2]));
+                    mx3 = fmaxf(mx3, __uint_as_float(sv[c + 3]));
+                }
+                const float mx = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
+                // reference hand-off: m_ref(n-1) from the previous team's warp of the same rows, lazy raise,
+                // m_ref(n) to the next team
+                float m_prev = -INFINITY;
+                if (n > 0) {
+                    mbar_wait(bar(kBarRef + 4 * tp + w), ((n - 1) >> 2) & 1);
+                    m_prev = xm[tp * kTileM + rl];
+                }
+                const bool need = n > 0 && mx > m_prev + thr;
+                const float m_new = n == 0 ? mx : (need ? mx : m_prev);
+                if (!last) {
+                    xm[t * kTileM + rl] = m_new;
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(bar(kBarRef + 4 * t + w));
+                }
+                //@T (n < 12 ? 34 + (n >> 2) * 5 : 63)
+                if (m_new != m_mine) {  // this thread's own row sum follows the reference
+                    l_mine *= m_mine == -INFINITY ? 0.f : ex2((m_mine - m_new) * c2);
+                    m_mine = m_new;
+                }
+                if (__any_sync(0xffffffffu, need)) {
+                    // O holds sub-units < n relative to m_prev: wait for P.V of sub-unit n-1, rescale this row.
+                    // P.V of sub-unit n cannot start before this thread releases P_n below.
+                    // A parity wait is only sound for the current or the preceding phase.  This thread last observed
+                    // this barrier (if at all) several phases ago, but its own P guard at sub-unit n-4 has seen P.V of
+                    // n-8 complete, hence also n-9: waiting for n-5 and then n-1 walks the phases one by one.
+                    if (n - 1 >= kTeams) mbar_wait(bar(kBarPFree + tp), (((n - 1) >> 2) & 1) ^ 1);
+                    mbar_wait(bar(kBarPFree + tp), ((n - 1) >> 2) & 1);
+                    tc_fence_after();
+                    const float alpha = need ? (m_prev == -INFINITY ? 0.f : ex2((m_prev - m_new) * c2)) : 1.f;
+#pragma unroll 1
+                    for (int c0 = 0; c0 < kD; c0 += 16) {
+                        uint32_t o[16];
+                        asm volatile(
+                            "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                            : "=r"(o[0]), "=r"(o[1]), "=r"(o[2]), "=r"(o[3]), "=r"(o[4]), "=r"(o[5]), "=r"(o[6]), "=r"(o[7]),
+                              "=r"(o[8]), "=r"(o[9]), "=r"(o[10]), "=r"(o[11]), "=r"(o[12]), "=r"(o[13]), "=r"(o[14]), "=r"(o[15])
+                            : "r"(tmem + lane_addr + c0));
+                        tmem_wait_ld();
+#pragma unroll
+                        for (int c = 0; c < 16; ++c) o[c] = __float_as_uint(__uint_as_float(o[c]) * alpha);
+                        D2SD_TMEM_ST16(tmem + lane_addr + c0, o);
+                    }
                     tmem_wait_st();
                     tc_fence_before();
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive(bar(kBarPFull + 4 * s + q - 1));
-                    //@T (n < 8 && q == 1 ? 35 + 5 * (n >> 1) : 63)
                 }
-                uint32_t p[16];
-                float t0 = 0.f, t1 = 0.f, t2 = 0.f, t3 = 0.f;
+                // the P buffer is free once P.V of sub-unit n-4 has completed
+                if (n >= kTeams) mbar_wait(bar(kBarPFree + t), par ^ 1);
+                // a row with every key so far masked has m_ref = -inf: exp2(-inf - 0) = 0, not NaN
+                const float ms = m_new == -INFINITY ? 0.f : m_new * c2;
+                float sum0 = 0.f, sum1 = 0.f;
+                // P[128 x 64] bf16 = 32 TMEM columns, written in two 32-key pieces (the exponentials replace the
+                // scores in place: 64 + 16 live registers)
 #pragma unroll
-                for (int c = 0; c < 16; c += 2) {
-                    t0 += ev[2 * c]; t1 += ev[2 * c + 1]; t2 += ev[2 * c + 2]; t3 += ev[2 * c + 3];
-                    p[c] = pack2_bf16(ev[2 * c], ev[2 * c + 1]);
-                    p[c + 1] = pack2_bf16(ev[2 * c + 2], ev[2 * c + 3]);
+                for (int q = 0; q < 2; ++q) {
+#pragma unroll
+                    for (int c = 0; c < 32; ++c)
+                        sv[q * 32 + c] = __float_as_uint(ex2_ordered(__uint_as_float(sv[q * 32 + c]) * c2 - ms));
+                    uint32_t p[16];
+                    float t0 = 0.f, t1 = 0.f, t2 = 0.f, t3 = 0.f;
+#pragma unroll
+                    for (int c = 0; c < 16; c += 2) {
+                        const float e0 = __uint_as_float(sv[q * 32 + 2 * c]), e1 = __uint_as_float(sv[q * 32 + 2 * c + 1]);
+                        const float e2 = __uint_as_float(sv[q * 32 + 2 * c + 2]), e3 = __uint_as_float(sv[q * 32 + 2 * c + 3]);
+                        t0 += e0; t1 += e1; t2 += e2; t3 += e3;
+                        p[c] = pack2_bf16(e0, e1);
+                        p[c + 1] = pack2_bf16(e2, e3);
+                    }
+                    sum0 += t0 + t1;
+                    sum1 += t2 + t3;
+                    D2SD_TMEM_ST16(pbuf + q * 16, p);
                 }
-                sum0 += t0 + t1;
-                sum1 += t2 + t3;
-                D2SD_TMEM_ST16(pbuf + q * 16, p);
+                l_mine += sum0 + sum1;
+                tmem_wait_st();
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar(kBarPFull + t));
+                //@T (n < 12 ? 36 + (n >> 2) * 5 : 63)
             }
-            l_mine += sum0 + sum1;
-            tmem_wait_st();
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(bar(kBarPFull + 4 * s + 3));
-            //@T (n < 8 ? 36 + 5 * (n >> 1) : 63)
         }
-        // ---- epilogue: the two teams' row sums meet at the final reference; the normalised state leaves the
+        n_sub = n;
+        // ---- epilogue: the four teams' row sums meet at the final reference; the normalised state leaves the
         // CTA straight from registers through a per-warp transpose in shared memory (the rings are free):
-        // thread (team g, w, lane) holds columns 64g..64g+63 of row w*32+lane, the warp writes them as 256-byte
-        // runs.  A group with a single chunk writes its rows to `out` directly: no exchange at all. ----
-        if (warp_active && N > 0 && ((N - 1) & 1) == g) xm[g * kTileM + rl] = m_mine;  // owner of the last unit
+        // thread (team t, w, lane) holds columns 32t..32t+31 of row w*32+lane, the warp writes them as whole
+        // 32-byte sectors.  A group with a single chunk writes its rows to `out` directly: no exchange. ----
+        const int t_last = (n_sub - 1) & 3;
+        if (warp_active && n_sub > 0 && t_last == t) xm[t * kTileM + rl] = m_mine;  // owner of the last sub-unit
         mbar_wait(bar(kBarAllDone), 0);  // every MMA done: O is final, the rings are free
         //@T 56
-        named_bar_sync(9, 256);
-        const float m_fin = N > 0 ? xm[((N - 1) & 1) * kTileM + rl] : -INFINITY;
+        named_bar_sync(9, 512);
+        const float m_fin = n_sub > 0 ? xm[t_last * kTileM + rl] : -INFINITY;
         if (m_fin != m_mine) l_mine *= m_mine == -INFINITY ? 0.f : ex2((m_mine - m_fin) * c2);
+        named_bar_sync(10, 512);  // everybody has read the final reference: the row sums take its place
         float* xl = reinterpret_cast<float*>(smem_gen + kOffXL);
-        xl[g * kTileM + rl] = l_mine;
-        named_bar_sync(10, 256);
-        const float l_tot = l_mine + xl[(g ^ 1) * kTileM + rl];
+        xl[t * kTileM + rl] = l_mine;
+        named_bar_sync(9, 512);
+        const float l_tot = (xl[rl] + xl[kTileM + rl]) + (xl[2 * kTileM + rl] + xl[3 * kTileM + rl]);
         const float inv = l_tot > 0.f ? 1.f / l_tot : 0.f;  // l = 0: every key of the chunk masked, or no key at all
         const float lse_v = l_tot > 0.f ? m_fin * pl.sm_scale + logf(l_tot) : -INFINITY;
         //@T 57
@@ -901,45 +939,39 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
         const bool row_ok = rl < wk.rows;
         const size_t prow0 = (size_t)wk.group * pl.grp_rows + (size_t)wk.chunk * kTileM;
         if (warp_active) {
-            // [32 rows][256 B] of fp32 (direct output) or [32 rows][128 B] of bf16 pairs (partial state), 16-byte
-            // chunks XOR-swizzled by the row
-            const uint32_t region = smem + kOffK + (uint32_t)warp * 8192u;
+            // per-warp staging: [32 rows][128 B] of fp32 (direct output) or [32 rows][64 B] of bf16 pairs (partial
+            // state), 16-byte chunks XOR-swizzled by the row
+            const uint32_t region = smem + kOffK + (uint32_t)warp * 4096u;
             const int G = pl.G;
+            uint32_t ov[32];
             tc_fence_after();
+            if (n_sub > 0) {
+                D2SD_TMEM_LD32(tmem + lane_addr + t * 32, ov, 0);
+                tmem_wait_ld();
+            }
+#pragma unroll
+            for (int c = 0; c < 32; ++c) ov[c] = n_sub > 0 ? __float_as_uint(__uint_as_float(ov[c]) * inv) : 0u;
             if (direct) {
 #pragma unroll
-                for (int c0 = 0; c0 < 64; c0 += 32) {
-                    uint32_t ov[32];
-                    if (N > 0) {
-                        D2SD_TMEM_LD32(tmem + lane_addr + g * 64 + c0, ov, 0);
-                        tmem_wait_ld();
-                    }
-#pragma unroll
-                    for (int c = 0; c < 32; c += 4) {
-                        const uint32_t chunk = (uint32_t)((c0 + c) >> 2) ^ ((uint32_t)lane & 15u);
-                        float f0 = 0.f, f1 = 0.f, f2 = 0.f, f3 = 0.f;
-                        if (N > 0) {
-                            f0 = __uint_as_float(ov[c]) * inv; f1 = __uint_as_float(ov[c + 1]) * inv;
-                            f2 = __uint_as_float(ov[c + 2]) * inv; f3 = __uint_as_float(ov[c + 3]) * inv;
-                        }
-                        asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(region + (uint32_t)lane * 256u + chunk * 16u),
-                                     "f"(f0), "f"(f1), "f"(f2), "f"(f3)
-                                     : "memory");
-                    }
+                for (int c = 0; c < 32; c += 4) {
+                    const uint32_t chunk = (uint32_t)(c >> 2) ^ ((uint32_t)lane & 7u);
+                    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(region + (uint32_t)lane * 128u + chunk * 16u),
+                                 "r"(ov[c]), "r"(ov[c + 1]), "r"(ov[c + 2]), "r"(ov[c + 3])
+                                 : "memory");
                 }
                 __syncwarp();
-#pragma unroll 4
-                for (int it = 0; it < 16; ++it) {
-                    const int row = it * 2 + (lane >> 4), ck = lane & 15;
+#pragma unroll 1
+                for (int it = 0; it < 8; ++it) {
+                    const int row = it * 4 + (lane >> 3), ck = lane & 7;
                     float4 v;
                     asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];"
                                  : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
-                                 : "r"(region + (uint32_t)row * 256u + (uint32_t)((ck ^ (row & 15)) * 16)));
+                                 : "r"(region + (uint32_t)row * 128u + (uint32_t)((ck ^ (row & 7)) * 16)));
                     const int r = w * 32 + row;  // row of the tile
                     if (r >= wk.rows) continue;
-                    const int col = g * 64 + ck * 4;
-                    const int ra = wk.row_base + r, t = ra / G;
-                    const size_t orow = ((size_t)wk.b * pl.T_cap + t) * pl.Hq + wk.g * G + (ra - t * G);
+                    const int col = t * 32 + ck * 4;
+                    const int ra = wk.row_base + r, tn = ra / G;
+                    const size_t orow = ((size_t)wk.b * pl.T_cap + tn) * pl.Hq + wk.g * G + (ra - tn * G);
                     if (dbg_rows) {
                         float* d0 = dbg_rows + orow * (kD + 1) + col;
                         d0[0] = v.x; d0[1] = v.y; d0[2] = v.z; d0[3] = v.w;
@@ -952,45 +984,33 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
                 }
             } else {
 #pragma unroll
-                for (int c0 = 0; c0 < 64; c0 += 32) {
-                    uint32_t ov[32];
-                    if (N > 0) {
-                        D2SD_TMEM_LD32(tmem + lane_addr + g * 64 + c0, ov, 0);
-                        tmem_wait_ld();
-                    }
+                for (int c = 0; c < 32; c += 8) {  // 8 columns = one 16-byte chunk of bf16
+                    const uint32_t chunk = (uint32_t)(c >> 3) ^ ((uint32_t)(lane >> 1) & 3u);
+                    uint32_t pk[4];
 #pragma unroll
-                    for (int c = 0; c < 32; c += 8) {  // 8 columns = one 16-byte chunk of bf16
-                        const uint32_t chunk = (uint32_t)((c0 + c) >> 3) ^ ((uint32_t)lane & 7u);
-                        uint32_t pk[4] = {0u, 0u, 0u, 0u};
-                        if (N > 0) {
-#pragma unroll
-                            for (int e = 0; e < 4; ++e)
-                                pk[e] = pack2_bf16(__uint_as_float(ov[c + 2 * e]) * inv, __uint_as_float(ov[c + 2 * e + 1]) * inv);
-                        }
-                        asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(region + (uint32_t)lane * 128u + chunk * 16u),
-                                     "r"(pk[0]), "r"(pk[1]), "r"(pk[2]), "r"(pk[3])
-                                     : "memory");
-                    }
+                    for (int e = 0; e < 4; ++e) pk[e] = pack2_bf16(__uint_as_float(ov[c + 2 * e]), __uint_as_float(ov[c + 2 * e + 1]));
+                    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(region + (uint32_t)lane * 64u + chunk * 16u),
+                                 "r"(pk[0]), "r"(pk[1]), "r"(pk[2]), "r"(pk[3])
+                                 : "memory");
                 }
                 __syncwarp();
-#pragma unroll 4
-                for (int it = 0; it < 8; ++it) {
-                    const int row = it * 4 + (lane >> 3), ck = lane & 7;
+#pragma unroll 1
+                for (int it = 0; it < 4; ++it) {
+                    const int row = it * 8 + (lane >> 2), ck = lane & 3;
                     uint4 v;
                     asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];"
                                  : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w)
-                                 : "r"(region + (uint32_t)row * 128u + (uint32_t)((ck ^ (row & 7)) * 16)));
+                                 : "r"(region + (uint32_t)row * 64u + (uint32_t)((ck ^ ((row >> 1) & 3)) * 16)));
                     const int r = w * 32 + row;  // row of the tile
-                    if (r < wk.rows) *reinterpret_cast<uint4*>(a.part_o16 + (prow0 + r) * kD + g * 64 + ck * 8) = v;
+                    if (r < wk.rows) *reinterpret_cast<uint4*>(a.part_o16 + (prow0 + r) * kD + t * 32 + ck * 8) = v;
                 }
             }
-            if (g == 0 && row_ok) {
+            if (t == 0 && row_ok) {
                 if (!direct) {
                     a.part_lse[prow0 + rl] = lse_v;
                 } else {
-                    const int G = pl.G;
-                    const int ra = wk.row_base + rl, t = ra / G;
-                    const size_t orow = ((size_t)wk.b * pl.T_cap + t) * pl.Hq + wk.g * G + (ra - t * G);
+                    const int ra = wk.row_base + rl, tn = ra / G;
+                    const size_t orow = ((size_t)wk.b * pl.T_cap + tn) * pl.Hq + wk.g * G + (ra - tn * G);
                     if (dbg_rows) dbg_rows[orow * (kD + 1) + kD] = lse_v;
                     else if (a.lse) a.lse[orow] = lse_v;
                 }
@@ -1000,7 +1020,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
             // ---- publish this CTA's partial state, wait for the group, merge this CTA's share of rows ----
             const unsigned expected = (unsigned)wk.n_chunks;
             unsigned* cnt = a.counters + 2 * wk.group;  // [0] arrivals, [1] done
-            named_bar_sync(9, 256);  // every thread's partial-state writes happen before the leader's (cumulative) release
+            named_bar_sync(10, 512);  // every thread's partial-state writes happen before the leader's (cumulative) release
             //@T 58
             unsigned done_before = 0;
             int ok = 1;
@@ -1021,11 +1041,12 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
                         }
                     }
                 } while (seen < expected);
+                __threadfence();  // acquire side: the states are read with ordinary loads behind the barrier below
                 // this CTA is past the wait: count it out now, the round trip hides behind the merge
                 done_before = atomicAdd(cnt + 1, 1u);
                 xl[0] = __int_as_float(ok);
             }
-            named_bar_sync(10, 256);
+            named_bar_sync(9, 512);
             //@T 59
             if (__float_as_int(xl[0]))
                 merge_rows(pl, a, dbg_rows, wk, warp, lane);
@@ -1042,7 +1063,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
 
     tc_fence_before();
     __syncthreads();
-    if (warp == 10) {
+    if (warp == 18) {
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(kTmemCols) : "memory");
     }
     //@T 61
