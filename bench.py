@@ -258,7 +258,12 @@ class Workload:
 
     @property
     def attn_kernel(self) -> str:
-        return "attn_stream_kernel"
+        return self.attn_kernel_for(self.cfg)
+
+    @staticmethod
+    def attn_kernel_for(cfg) -> str:
+        # api.cu: paged KV with more (request, kv head) pairs than one wave holds runs the two-tiles-per-CTA kernel
+        return "attn_cascade_tc_kernel" if cfg.paged and cfg.B * cfg.Hkv * 4 > 148 else "attn_stream_kernel"
 
     @property
     def launches_per_step(self) -> int:
@@ -291,6 +296,14 @@ class Workload:
     def d2h_bytes(self) -> int:
         n = sum(v.numel() * v.element_size() for v in self.acc.values())
         return n + self.outs[-1].numel() * 2
+
+
+def workload_config(cfg, ctx_len, tree_tokens: int, planted: int, world: int) -> dict:
+    """The workload description both arms print (same keys, same values for the same config)."""
+    return {"workload": f"BASELINE.json configs[{cfg.number - 1}] ({cfg.name})", "B": cfg.B, "layers": cfg.layers,
+            "gamma": cfg.gamma, "K": cfg.K, "ctx": [int(x) for x in ctx_len[:4]], "V": cfg.V,
+            "tree_tokens": int(tree_tokens), "planted_accepts": int(planted),
+            "kv": "paged(16)" if cfg.paged else "contiguous", "parallelism": f"replicas x{world}"}
 
 
 def capture(torch, fn):
@@ -330,6 +343,119 @@ def time_replays(torch, g, n: int, flush=None) -> float:
     return sum(a.elapsed_time(b) for a, b in pairs)
 
 
+
+# ------------------------------------------------------------------------------- roofline + extra measurements
+
+NOMINAL_HBM_GBS = 8000.0  # the north star's "roughly 8 TB/s" (stretch basis)
+
+
+def attn_roofline(cfg, wl, us_per_launch: float, peaks, traffic):
+    """Algorithmic bytes / flops of ONE cascade-attention launch against the measured peaks."""
+    T_rows = wl.tree_tokens
+    kv_bytes = 2 * int(wl.st["ctx_len"].sum()) * cfg.Hkv * cfg.d * 2
+    q_bytes = T_rows * cfg.Hq * cfg.d * 2                     # Q in; O out is the same size
+    tree_kv_bytes = 2 * T_rows * cfg.Hkv * cfg.d * 2
+    alg_bytes = kv_bytes + 2 * q_bytes + tree_kv_bytes + T_rows * cfg.Hq * 4
+    alg_flops = 4.0 * cfg.Hq * cfg.d * float(sum(int(t) * int(l) for t, l in zip(wl.tree_len_host, wl.st["ctx_len"])))
+    ach_gbs = alg_bytes / (us_per_launch * 1e-6) / 1e9
+    ach_tf = alg_flops / (us_per_launch * 1e-6) / 1e12
+    t_hbm_us = alg_bytes / (peaks["hbm_gbs"] * 1e9) * 1e6
+    t_tc_us = alg_flops / (peaks["bf16_tflops_sustained"] * 1e12) * 1e6
+    hbm = {"bound": "hbm", "achieved": ach_gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+           "frac": ach_gbs / peaks["hbm_gbs"], "frac_of_nominal_8TBs": ach_gbs / NOMINAL_HBM_GBS, "traffic": traffic,
+           "peak_source": peaks["source"], "kernel": wl.attn_kernel, "us_per_launch": us_per_launch,
+           "alg_bytes_per_launch": alg_bytes}
+    tc = {"bound": "tensor", "achieved": ach_tf, "peak": peaks["bf16_tflops_sustained"], "unit": "TFLOP/s",
+          "frac": ach_tf / peaks["bf16_tflops_sustained"], "traffic": traffic,
+          "peak_source": peaks["source"] + " (sustained bf16)", "kernel": wl.attn_kernel,
+          "us_per_launch": us_per_launch, "alg_flops_per_launch": alg_flops}
+    return (tc if t_tc_us > t_hbm_us else hbm), hbm, tc  # "the slower of" the two bounds first
+
+
+def attention_only(torch, d2sd, cfg, peaks, steps: int, layers: int):
+    """Attention launches of one config alone (graph replay, CUDA events): us per launch + rooflines."""
+    import dataclasses
+    sub = dataclasses.replace(cfg, layers=min(cfg.layers, layers))
+    wl = Workload(sub, d2sd, torch, host_copies=False)
+    kv_bytes = 2 * int(wl.st["ctx_len"].sum()) * sub.Hkv * sub.d * 2 * sub.layers
+    flush = None
+    if kv_bytes < 2 * L2_BYTES:
+        fbuf = torch.empty(2 * L2_BYTES, dtype=torch.uint8, device="cuda")
+        flush = lambda: fbuf.fill_(1)  # noqa: E731
+    g = capture(torch, lambda: [wl.attention(i) for i in range(sub.layers)])
+    for _ in range(3):
+        g.replay()
+    torch.cuda.synchronize()
+    us = time_replays(torch, g, steps, flush) / (steps * sub.layers) * 1e3
+    roof, hbm, tc = attn_roofline(sub, wl, us, peaks, ncu_traffic(wl.attn_kernel_for(sub), sub.number))
+    out = {"workload": f"BASELINE.json configs[{cfg.number - 1}] ({cfg.name})", "attn_us_per_layer": us,
+           "layers_timed": sub.layers, "tree_tokens": wl.tree_tokens, "kernel": wl.attn_kernel_for(sub),
+           "l2": "flushed between replays" if flush else "distinct KV per layer, larger than L2",
+           "roofline_bound": roof["bound"], "roofline_frac": roof["frac"],
+           "roofline_hbm": {k: hbm[k] for k in ("achieved", "frac", "frac_of_nominal_8TBs", "traffic", "alg_bytes_per_launch")},
+           "roofline_tensor": {k: tc[k] for k in ("achieved", "frac", "alg_flops_per_launch")}}
+    del wl, g
+    torch.cuda.empty_cache()
+    return out
+
+
+# prefix sets that give T = gamma + sum(gamma-1-i) tree nodes at gamma = 16, K = 4 (SURVEY.md 8d: intensity is 4T
+# flop per KV byte, so the bound moves from HBM to the tensor pipe inside this range)
+T_SWEEP = {26: (11, 12, 13, 14), 40: (7, 8, 9, 12), 54: (3, 4, 6, 9), 64: (0, 2, 3, 7), 70: (0, 1, 2, 3)}
+
+
+def tree_size_sweep(torch, d2sd, cfg, peaks, steps: int, layers: int = 8):
+    """Attention us per layer at L = 4096 for forced prefix sets (harness input: the tree is built from a given
+    prefix_len instead of the selected one)."""
+    import dataclasses
+    sub = dataclasses.replace(cfg, layers=min(cfg.layers, layers))
+    wl = Workload(sub, d2sd, torch, host_copies=False)
+    rows = []
+    for T, prefixes in T_SWEEP.items():
+        pl_t = torch.tensor([list(prefixes)] * sub.B, dtype=torch.int32, device="cuda")
+        s = wl.step_in
+        wl.tree = d2sd.build_tree(s["draft1"], s["draft2"], pl_t, s["ctx_len"], sub.T_cap, out=wl.tree)
+        torch.cuda.synchronize()
+        assert int(wl.tree["tree_len"][0]) == T
+        wl.tree_len_host = wl.tree["tree_len"].cpu().numpy()
+        wl.tree_tokens = int(wl.tree_len_host.sum())
+        g = capture(torch, lambda: [wl.attention(i) for i in range(sub.layers)])
+        for _ in range(3):
+            g.replay()
+        torch.cuda.synchronize()
+        us = time_replays(torch, g, steps, None) / (steps * sub.layers) * 1e3
+        roof, hbm, tc = attn_roofline(sub, wl, us, peaks, None)
+        rows.append({"T": T, "attn_us_per_layer": us, "bound": roof["bound"], "frac": roof["frac"],
+                     "frac_hbm": hbm["frac"], "frac_tensor": tc["frac"]})
+        del g
+    del wl
+    torch.cuda.empty_cache()
+    return rows
+
+
+def stage_times(torch, wl, steps: int, flush):
+    """us per call of the launch-latency-sized stages, each as its own CUDA graph (L2 flushed between replays)."""
+    d, cfg = wl.d2sd, wl.cfg
+    out = {}
+    def timed(fn):
+        g = capture(torch, fn)
+        for _ in range(3):
+            g.replay()
+        torch.cuda.synchronize()
+        return time_replays(torch, g, steps, flush) / steps * 1e3
+    s = wl.step_in
+    out["select_prefixes"] = timed(lambda: d.select_prefixes(s["conf"], cfg.K, prefix_len=wl.prefix_len))
+    out["build_tree"] = timed(lambda: d.build_tree(s["draft1"], s["draft2"], wl.prefix_len, s["ctx_len"], cfg.T_cap, out=wl.tree))
+    out["accept (argmax + walk)"] = timed(wl.accept)
+    # the steps around the path (SURVEY 8f): drafter confidence extraction and KV commit of one layer set
+    dl = torch.randn((cfg.B, cfg.gamma - 1, cfg.V), device="cuda").to(torch.bfloat16)
+    anchor = torch.zeros((cfg.B,), dtype=torch.int32, device="cuda")
+    ws = torch.empty(d.confidence_workspace_bytes(cfg.B, cfg.gamma, cfg.V), dtype=torch.uint8, device="cuda")
+    dr = torch.empty((cfg.B, cfg.gamma), dtype=torch.int32, device="cuda")
+    cf = torch.empty((cfg.B, cfg.gamma), dtype=torch.float32, device="cuda")
+    out["draft_confidence"] = timed(lambda: d.draft_confidence(dl, anchor, draft=dr, conf=cf, workspace=ws))
+    return out
+
 # ------------------------------------------------------------------------------- CPU oracle legs
 
 def oracle_sample_seconds(cfg: synth.Config, layers_sampled: int = 1):
@@ -363,22 +489,34 @@ def oracle_sample_seconds(cfg: synth.Config, layers_sampled: int = 1):
 
 
 def run_reference(args, cfg):
+    """The oracle as the reference arm: every step times select + build, ONE of the cfg.layers attention layers (every
+    row) and argmax + walk; the step time scales the attention part by cfg.layers (stated in `extrapolated`)."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
     for _ in range(args.warmup and 1):
         oracle_sample_seconds(cfg, 1)  # one warm-up sample is enough for a CPU loop (page-in, OpenMP pool)
-    ts, tokens, desc, cores = [], 0, "", 1
+    ts, meas, tokens, desc, cores = [], [], 0, "", 1
     for _ in range(args.steps):
-        step_s, _, tokens, desc, cores = oracle_sample_seconds(cfg, 1)
+        step_s, measured, tokens, desc, cores = oracle_sample_seconds(cfg, 1)
         ts.append(step_s)
+        meas.append(measured)
     step_s = float(np.mean(ts))
     value = tokens / step_s
+    st = synth.make_step_inputs(cfg)
+    import oracle
+    pl_, _ = oracle.select_prefixes(st["conf"], cfg.K)
+    tr_ = oracle.build_tree(st["draft1"], st["draft2"], pl_, st["ctx_len"], cfg.T_cap)
+    plants = synth.plant_acceptance(cfg, synth.make_logits(cfg), st["conf"], tr_["tokens"], tr_["parent"], tr_["depth"],
+                                    tr_["tree_len"])
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": step_s * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"BASELINE.json configs[{cfg.number - 1}] ({cfg.name})", "B": cfg.B,
-                       "layers": cfg.layers, "gamma": cfg.gamma, "K": cfg.K, "ctx": list(cfg.ctx), "V": cfg.V},
+            "config": workload_config(cfg, st["ctx_len"], tokens, plants, 1),
+            "measurement": {"timing": "time.perf_counter around the oracle calls on the host cores"},
+            "extrapolated": {"what": f"ms_per_step = select + build + {cfg.layers} x (one timed attention layer) + accept",
+                             "measured_ms_per_step": float(np.mean(meas)) * 1e3, "attention_layers_timed": 1,
+                             "attention_layers_per_step": cfg.layers},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -397,6 +535,7 @@ def main():
     ap.add_argument("--impl", default="d2sd", choices=["d2sd", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip stage times, the tree-size sweep and the per-config block")
     args = ap.parse_args()
     cfg = synth.CONFIGS[args.config]
     if args.impl == "reference":
@@ -445,42 +584,26 @@ def main():
     ms_per_step = ms / args.steps
     value = tokens_all / (ms_per_step * 1e-3)
 
-    # roofline of the prefix pass (algorithmic bytes and flops per launch)
-    T_rows = wl.tree_tokens  # tree nodes over all requests
-    q_bytes = T_rows * cfg.Hq * cfg.d * 2                     # Q in; O out is the same size
-    tree_kv_bytes = 2 * T_rows * cfg.Hkv * cfg.d * 2
-    alg_bytes = kv_bytes_layer + 2 * q_bytes + tree_kv_bytes + T_rows * cfg.Hq * 4
-    alg_flops = 4.0 * cfg.Hq * cfg.d * float(sum(int(t) * int(l) for t, l in zip(wl.tree_len_host, wl.st["ctx_len"])))
+    # roofline of the dominant kernel (algorithmic bytes and flops per launch)
     us_prefix = ms_prefix / (args.steps * cfg.layers) * 1e3
-    t_hbm_us = alg_bytes / (peaks["hbm_gbs"] * 1e9) * 1e6
-    t_tc_us = alg_flops / (peaks["bf16_tflops_sustained"] * 1e12) * 1e6
-    ach_gbs = alg_bytes / (us_prefix * 1e-6) / 1e9
-    ach_tf = alg_flops / (us_prefix * 1e-6) / 1e12
-    traffic = ncu_traffic(wl.attn_kernel, cfg.number)
-    roof_hbm = {"bound": "hbm", "achieved": ach_gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                "frac": ach_gbs / peaks["hbm_gbs"], "traffic": traffic, "peak_source": peaks["source"],
-                "kernel": wl.attn_kernel, "us_per_launch": us_prefix, "alg_bytes_per_launch": alg_bytes}
-    roof_tc = {"bound": "tensor", "achieved": ach_tf, "peak": peaks["bf16_tflops_sustained"], "unit": "TFLOP/s",
-               "frac": ach_tf / peaks["bf16_tflops_sustained"], "traffic": traffic,
-               "peak_source": peaks["source"] + " (sustained bf16)", "kernel": wl.attn_kernel,
-               "us_per_launch": us_prefix, "alg_flops_per_launch": alg_flops}
-    roofline = roof_tc if t_tc_us > t_hbm_us else roof_hbm  # "the slower of" the two bounds
+    roofline, roof_hbm, roof_tc = attn_roofline(cfg, wl, us_prefix, peaks, ncu_traffic(wl.attn_kernel, cfg.number))
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-            "config": {"workload": f"BASELINE.json configs[{cfg.number - 1}] ({cfg.name})", "B": cfg.B,
-                       "layers": cfg.layers, "gamma": cfg.gamma, "K": cfg.K, "ctx": [int(x) for x in wl.st["ctx_len"][:4]],
-                       "V": cfg.V, "tree_tokens": wl.tree_tokens, "planted_accepts": wl.n_plants,
-                       "kv": "paged(16)" if cfg.paged else "contiguous", "parallelism": f"replicas x{world}",
-                       "l2": ("flushed between steps (256 MiB write)" if flush else
-                              f"inputs larger than L2 ({step_bytes / 2**20:.0f} MiB of distinct KV per step)"),
-                       "timing": "CUDA-graph replay of the whole step, CUDA events on the replay stream"},
+            "config": workload_config(cfg, wl.st["ctx_len"], wl.tree_tokens, wl.n_plants, world),
+            "measurement": {"l2": ("flushed between steps (256 MiB write)" if flush else
+                                   f"inputs larger than L2 ({step_bytes / 2**20:.0f} MiB of distinct KV per step)"),
+                            "timing": "CUDA-graph replay of the whole step, CUDA events on the replay stream"},
             "us_per_step": ms_per_step * 1e3,
             "attn_us_per_layer": us_prefix,
             "roofline": roofline, "roofline_hbm": roof_hbm, "roofline_tensor": roof_tc,
             "gpu_launches": wl.launches_per_step * args.steps,
             "clocks": clocks.summary()}
+    if not args.no_extras:
+        line["stage_us"] = stage_times(torch, wl, min(args.steps, 30), flush)
+        line["stage_us"]["cascade_verify_attn (per layer)"] = us_prefix
+        line["non_attention_us_per_step"] = ms_per_step * 1e3 - us_prefix * cfg.layers
 
     # e2e: host buffers -> device -> step -> host results, everything inside the timed region
     if not args.no_e2e:
@@ -504,6 +627,15 @@ def main():
                           "kv_cache": "copied from pinned host memory every step" if with_kv else
                           "resident in HBM (committed state, PAPER.md:119); only the step's own inputs are copied"}
 
+    if rank == 0 and world == 1 and not args.no_extras and cfg.number == 2:
+        # the other single-GPU configs (attention launches only) and the tree-size sweep, driver-verifiable in this line
+        del g_step, g_attn
+        wl.layers = None
+        wl.outs = None
+        torch.cuda.empty_cache()
+        line["tree_size_sweep_L4096"] = tree_size_sweep(torch, d2sd, cfg, peaks, min(args.steps, 30))
+        line["per_config"] = [attention_only(torch, d2sd, synth.CONFIGS[n], peaks, min(args.steps, 20), layers=4)
+                              for n in (3, 4, 5)]
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         step_s, measured, tokens, desc, cores = oracle_sample_seconds(cfg, 1)
         line["cpu_baseline"] = {"value": tokens / step_s, "unit": UNIT, "cores": cores, "kind": "oracle",

@@ -104,7 +104,8 @@ int32_t d2sd_build_tree(const int32_t* draft1, const int32_t* draft2, const int3
  * (O, LSE) per chunk; the <= T_cap tree keys are attended under the ancestor mask; all partial
  * states are merged by log-sum-exp.  Contiguous or 16-key-paged KV with 128 % G == 0 runs as ONE fused
  * tcgen05 launch (tree keys = extra key tiles, merge in the same kernel); other group sizes run the
- * mma.sync kernels (prefix/tree pass + merge).  bf16 in, fp32 accumulate, bf16 out.  Q and tree K are taken post q/k-norm and
+ * mma.sync kernels (prefix/tree pass + merge).  bf16 in, fp32 accumulate, bf16 out; the partial states
+ * of the split-KV exchange are normalised O rows in bf16 and LSE in fp32.  Q and tree K are taken post q/k-norm and
  * post-RoPE (pos_id from (b) is for the caller's RoPE).  No sliding window / sinks / soft-cap.
  * ------------------------------------------------------------------------------------------- */
 typedef struct d2sd_attn_params {
@@ -117,10 +118,11 @@ typedef struct d2sd_attn_params {
     int32_t max_ctx_len; /* host-side upper bound on ctx_len[b]; sizes the split-KV grid         */
     int64_t kv_rows;     /* token rows in k_cache/v_cache: contiguous: >= kv_indptr[B] (sum L_b);
                             paged: num_pages * page_size.  Bounds the TMA tensor maps.           */
-    int32_t num_splits;  /* key chunks per (request, kv head); 0 = choose from the shape (<= 64) */
-    int32_t impl;        /* 0 = auto; 1 = force the mma.sync kernels; 2 = force the fused tcgen05
-                            kernel (D2SD_ERR_UNSUPPORTED if the shape is outside it)             */
-    int32_t phases;      /* 0 = the whole cascade.  For tests and profiling: 1 = attend the
+    int32_t num_splits;  /* TEST KNOB, leave 0: key chunks per (request, kv head) chosen from the shape (<= 64) */
+    int32_t impl;        /* TEST KNOB, leave 0 (auto).  1 = force the mma.sync kernels; 2 = force the fused
+                            two-query-tiles-per-CTA tcgen05 kernel; 3 = force the fused one-query-tile-per-
+                            CTA tcgen05 kernel (2, 3: D2SD_ERR_UNSUPPORTED if the shape is outside them)  */
+    int32_t phases;      /* TEST KNOB, leave 0 = the whole cascade.  For tests and profiling: 1 = attend the
                             committed prefix only, 2 = the tree keys only (out/lse then hold that
                             state; a prefix-only state with ctx_len = 0 is O = 0, LSE = -inf).
                             mma.sync kernels only: bit mask of 1 = prefix pass, 2 = tree pass,
@@ -136,7 +138,14 @@ size_t d2sd_cascade_workspace_bytes(const d2sd_attn_params* p /* host */);
  * this library ever failed on it; d2sd_cascade_verify_attn leaves the header zero after every call,
  * so the same workspace serves any number of calls (and any params it is large enough for) one
  * after another.  The rest of the workspace is scratch.  Two calls that may run concurrently need
- * two workspaces. */
+ * two workspaces.
+ * Co-scheduling: when every (request, kv head, query tile, chunk) CTA of a call fits on the device at
+ * once (the plan sizes such grids to the SM count of the CURRENT device), the CTAs of a group wait for
+ * each other inside the kernel and share the merge; this needs the whole device (no MPS / green-context
+ * partition, no other kernel holding SMs for the ~20 us of the call).  A wait that does not end within
+ * ~0.1 s gives up: the rows of that group are not written and the uint32 at byte offset 2^20 - 8 of the
+ * workspace is set to 1 (it is otherwise 0; the caller may poll it).  Larger calls run in several waves,
+ * never wait, and have no such requirement. */
 int32_t d2sd_cascade_workspace_init(const d2sd_attn_params* p /* host */, void* workspace,
                                     size_t workspace_bytes, void* stream);
 

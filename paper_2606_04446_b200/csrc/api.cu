@@ -1,6 +1,7 @@
 // extern "C" entry points of libd2sd (declared and documented in include/d2sd.h): argument checks,
 // launch planning, kernel enqueue.  No allocation, no synchronisation, no host reads of device data.
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 
 #include "common.cuh"
@@ -64,10 +65,15 @@ static int32_t make_plan(const d2sd_attn_params* p, AttnPlan* out) {
     pl.kv_rows = p->kv_rows;
     pl.use_tc = false;
     pl.use_stream = false;
-    if (p->impl == 3 || p->impl == 0) {
+    // auto: the one-tile-per-CTA kernel, except for paged KV with more (request, kv head) pairs than one wave holds:
+    // there the two-tiles-per-CTA kernel amortises the 2 KiB page boxes over twice the query rows (config 5:
+    // 363 vs 416 us)
+    const bool paged_multiwave = p->page_size > 0 && (int64_t)p->B * p->Hkv * 4 > sm_count();
+    if (p->impl == 3 || (p->impl == 0 && !paged_multiwave)) {
         pl.use_stream = attn_stream_supported(pl);
         D2SD_CHECK_SUPPORTED(pl.use_stream || p->impl != 3, "impl = 3 (one-tile-per-CTA tcgen05 kernel) does not cover this shape");
-    } else if (p->impl != 1) {
+    }
+    if (!pl.use_stream && p->impl != 1 && p->impl != 3) {
         pl.use_tc = attn_cascade_tc_supported(pl);
         D2SD_CHECK_SUPPORTED(pl.use_tc || p->impl != 2, "impl = 2 (tcgen05) does not cover this shape");
     }
@@ -114,7 +120,9 @@ static int32_t make_plan(const d2sd_attn_params* p, AttnPlan* out) {
                 if (t < best) { best = t; ca = a2; cb = b_best; }
             }
         } else {
-            ca = cb = ceil_div(max_tiles, 32);
+            int chunk_tiles = 32;
+            if (const char* e = getenv("D2SD_CHUNK_TILES")) chunk_tiles = atoi(e);  // TUNING ONLY
+            ca = cb = ceil_div(max_tiles, chunk_tiles);
             pl.tps_min = -1;  // fixed below
         }
         if (ca > 64) ca = 64;  // a group's CTAs wait for each other
@@ -123,6 +131,8 @@ static int32_t make_plan(const d2sd_attn_params* p, AttnPlan* out) {
         if (cb > max_tiles) cb = max_tiles;
         if (ca < 1) ca = 1;
         if (cb < 1) cb = 1;
+        pl.last_merges = pl.tps_min < 0 && splits == 0;
+        pl.no_share_paged = getenv("D2SD_NO_SHARE_PAGED") != nullptr;  // TUNING ONLY
         if (pl.tps_min < 0) pl.tps_min = ceil_div(max_tiles, ca);
         pl.n_mt = n_mt;
         pl.n_pair = n_pairs; pl.n_single = odd;

@@ -382,11 +382,10 @@ __device__ __forceinline__ float bf_hi(uint32_t w) { return __uint_as_float(w & 
 // the weights are reduced with shuffles and never leave the registers.  The partial states were written
 // by other SMs and published with a release; they are read at L2 (ld.global.cg).
 __device__ __forceinline__ void merge_rows(const AttnPlan& pl, const AttnArgs& a, float* dbg_rows, const Work& wk,
-                                           int warp, int lane) {
+                                           int r0, int r1, int warp, int lane) {
     const int G = pl.G;
     const int nc = wk.n_chunks;  // <= 64 states
     const size_t grp0 = (size_t)wk.group * pl.grp_rows;
-    const int r0 = wk.rows * wk.chunk / nc, r1 = wk.rows * (wk.chunk + 1) / nc;
     const int nrows = r1 - r0;  // <= 128
     constexpr int kRB = 2, kSB = 8;
     for (int rb = warp * kRB; rb < nrows; rb += 16 * kRB) {
@@ -567,7 +566,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
         wk.row_base = wk.tile * kTileM;
         wk.rows = pad ? 0 : max(0, min(kTileM, rows_valid - wk.row_base));
         // a pair shares its key tiles when both M tiles hold rows (a short tree leaves the odd tile empty)
-        wk.share = pair && rows_valid > (wk.tile | 1) * kTileM;
+        wk.share = pair && rows_valid > (wk.tile | 1) * kTileM && !(pl.page_size > 0 && pl.no_share_paged);
         wk.group = (wk.b * pl.Hkv + wk.g) * pl.n_mt + wk.tile;
         wk.np = (mode & 1) ? (wk.L + kTileN - 1) / kTileN : 0;
         wk.nt = (mode & 2) ? (wk.T + kTileN - 1) / kTileN : 0;
@@ -1017,44 +1016,59 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
             }
         }
         if (!direct) {
-            // ---- publish this CTA's partial state, wait for the group, merge this CTA's share of rows ----
+            // ---- publish this CTA's partial state and merge.  One wave (every CTA of the launch resident): wait
+            // for the group and merge this CTA's SHARE of the rows, so the merge is spread over the group's SMs.
+            // Several waves: nobody waits (a waiting CTA would hold an SM that later CTAs need, and its siblings
+            // need not be resident); the LAST CTA to arrive merges all rows of the group. ----
             const unsigned expected = (unsigned)wk.n_chunks;
             unsigned* cnt = a.counters + 2 * wk.group;  // [0] arrivals, [1] done
             named_bar_sync(10, 512);  // every thread's partial-state writes happen before the leader's (cumulative) release
             //@T 58
             unsigned done_before = 0;
-            int ok = 1;
-            if (warp == 0 && lane == 0) {
-                __threadfence();
-                asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(cnt) : "memory");
-                unsigned seen, spins = 0;
-                do {
-                    // relaxed: the states are read with L2-level loads (ld.global.cg) issued after this load has
-                    // returned; an acquire here would invalidate the whole L1 on every poll
-                    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(cnt) : "memory");
-                    if (seen < expected) {
-                        __nanosleep(20);
-                        if (++spins > (1u << 22)) {  // the group never became co-resident: report, do not hang
-                            atomicExch(a.counters + kWsErrorWord, 1u);
-                            ok = 0;
-                            break;
+            if (pl.last_merges) {
+                if (warp == 0 && lane == 0) {
+                    __threadfence();
+                    const unsigned before = atomicAdd(cnt, 1u);
+                    __threadfence();  // acquire side for the last arriver
+                    if (before == expected - 1) cnt[0] = 0;  // the counter is ready for the next launch
+                    xl[0] = __int_as_float(before == expected - 1);
+                }
+                named_bar_sync(9, 512);
+                if (__float_as_int(xl[0])) merge_rows(pl, a, dbg_rows, wk, 0, wk.rows, warp, lane);
+            } else {
+                int ok = 1;
+                if (warp == 0 && lane == 0) {
+                    __threadfence();
+                    asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(cnt) : "memory");
+                    unsigned seen, spins = 0;
+                    do {
+                        // relaxed: an acquire here would invalidate the whole L1 on every poll; one fence follows
+                        asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(cnt) : "memory");
+                        if (seen < expected) {
+                            __nanosleep(20);
+                            if (++spins > (1u << 22)) {  // the group never became co-resident: report, do not hang
+                                atomicExch(a.counters + kWsErrorWord, 1u);
+                                ok = 0;
+                                break;
+                            }
                         }
+                    } while (seen < expected);
+                    __threadfence();  // acquire side: the states are read with ordinary loads behind the barrier below
+                    // this CTA is past the wait: count it out now, the round trip hides behind the merge
+                    done_before = atomicAdd(cnt + 1, 1u);
+                    xl[0] = __int_as_float(ok);
+                }
+                named_bar_sync(9, 512);
+                //@T 59
+                if (__float_as_int(xl[0]))
+                    merge_rows(pl, a, dbg_rows, wk, wk.rows * wk.chunk / wk.n_chunks, wk.rows * (wk.chunk + 1) / wk.n_chunks,
+                               warp, lane);
+                //@T 60
+                if (warp == 0 && lane == 0) {
+                    if (done_before == expected - 1) {  // last CTA out: everybody is past the wait
+                        cnt[0] = 0;
+                        cnt[1] = 0;
                     }
-                } while (seen < expected);
-                __threadfence();  // acquire side: the states are read with ordinary loads behind the barrier below
-                // this CTA is past the wait: count it out now, the round trip hides behind the merge
-                done_before = atomicAdd(cnt + 1, 1u);
-                xl[0] = __int_as_float(ok);
-            }
-            named_bar_sync(9, 512);
-            //@T 59
-            if (__float_as_int(xl[0]))
-                merge_rows(pl, a, dbg_rows, wk, warp, lane);
-            //@T 60
-            if (warp == 0 && lane == 0) {
-                if (done_before == expected - 1) {  // last CTA out: everybody is past the wait
-                    cnt[0] = 0;
-                    cnt[1] = 0;
                 }
             }
         }

@@ -151,7 +151,8 @@ def test_accept_duplicate_siblings_prefers_trunk(d2sd, oracle):
 
 # ------------------------------------------------------------------------------------------ (c)
 
-IMPLS = [pytest.param(1, id="mma.sync"), pytest.param(0, id="auto-tcgen05")]
+IMPLS = [pytest.param(1, id="mma.sync"), pytest.param(0, id="auto-tcgen05"), pytest.param(2, id="two-tile"),
+         pytest.param(3, id="one-tile")]
 
 
 def _ramp_keys(kv, ctx_len, lo=0.25, hi=4.0):
@@ -174,7 +175,12 @@ def _attn_full_case(d2sd, oracle, cfg, q_scale=1.0, layer=0, pool_nan=False, ram
     kv = synth.make_kv_cache(cfg, st["ctx_len"], layer, pool_fill_nan=pool_nan)
     if ramp:
         _ramp_keys(kv, st["ctx_len"])
-    o, lse, dbg = gpu_attention(d2sd, cfg, st, tree, ti, kv, dbg=True, **kw)
+    try:
+        o, lse, dbg = gpu_attention(d2sd, cfg, st, tree, ti, kv, dbg=True, **kw)
+    except d2sd.D2sdError as e:
+        if kw.get("impl", 0) in (2, 3) and "does not cover" in str(e):
+            pytest.skip("a forced tcgen05 kernel does not cover this shape (auto falls back to mma.sync)")
+        raise
     args = (ti["q"], kv["k_cache"], kv["v_cache"], kv["kv_indptr"], kv["kv_indices"], kv["page_size"],
             st["ctx_len"], ti["tree_k"], ti["tree_v"], tree["mask"], tree["tree_len"])
     ro, rl = oracle.attention(*args, which="full")
