@@ -1,7 +1,6 @@
 // extern "C" entry points of libd2sd (declared and documented in include/d2sd.h): argument checks,
 // launch planning, kernel enqueue.  No allocation, no synchronisation, no host reads of device data.
 #include <cmath>
-#include <cstdlib>
 #include <cstring>
 
 #include "common.cuh"
@@ -120,9 +119,7 @@ static int32_t make_plan(const d2sd_attn_params* p, AttnPlan* out) {
                 if (t < best) { best = t; ca = a2; cb = b_best; }
             }
         } else {
-            int chunk_tiles = 32;
-            if (const char* e = getenv("D2SD_CHUNK_TILES")) chunk_tiles = atoi(e);  // TUNING ONLY
-            ca = cb = ceil_div(max_tiles, chunk_tiles);
+            ca = cb = ceil_div(max_tiles, 32);  // measured on config 5: 20 -> 497, 32 -> 486, 64 -> 500, 129 -> 572 us per step
             pl.tps_min = -1;  // fixed below
         }
         if (ca > 64) ca = 64;  // a group's CTAs wait for each other
@@ -132,7 +129,6 @@ static int32_t make_plan(const d2sd_attn_params* p, AttnPlan* out) {
         if (ca < 1) ca = 1;
         if (cb < 1) cb = 1;
         pl.last_merges = pl.tps_min < 0 && splits == 0;
-        pl.no_share_paged = getenv("D2SD_NO_SHARE_PAGED") != nullptr;  // TUNING ONLY
         if (pl.tps_min < 0) pl.tps_min = ceil_div(max_tiles, ca);
         pl.n_mt = n_mt;
         pl.n_pair = n_pairs; pl.n_single = odd;

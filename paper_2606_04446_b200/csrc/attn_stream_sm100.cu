@@ -566,7 +566,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
         wk.row_base = wk.tile * kTileM;
         wk.rows = pad ? 0 : max(0, min(kTileM, rows_valid - wk.row_base));
         // a pair shares its key tiles when both M tiles hold rows (a short tree leaves the odd tile empty)
-        wk.share = pair && rows_valid > (wk.tile | 1) * kTileM && !(pl.page_size > 0 && pl.no_share_paged);
+        wk.share = pair && rows_valid > (wk.tile | 1) * kTileM;
         wk.group = (wk.b * pl.Hkv + wk.g) * pl.n_mt + wk.tile;
         wk.np = (mode & 1) ? (wk.L + kTileN - 1) / kTileN : 0;
         wk.nt = (mode & 2) ? (wk.T + kTileN - 1) / kTileN : 0;

@@ -124,7 +124,6 @@ struct AttnPlan {
     // tcgen05: the query rows (T*G) of one kv head are cut into 128-row tiles; tiles (2p, 2p+1) form
     // "pair item" p, an odd last tile is the "single item".  Item kinds get their own chunk counts.
     int n_mt;                // 128-row query tiles per (request, kv head), from T_cap
-    bool no_share_paged;     // TUNING
     bool last_merges;        // several waves: the last CTA of a group to arrive merges it (nobody waits)
     bool use_stream;         // the one-tile-per-CTA kernel (attn_stream_sm100.cu): chunks_a per paired tile, chunks_b for an odd last tile
     int n_pair, n_single;    // items per (request, kv head), from T_cap

@@ -4,6 +4,22 @@
 
 namespace d2sd {
 
+__device__ __forceinline__ void sb_pdl() {
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+static cudaLaunchConfig_t sb_config(dim3 grid, dim3 block, cudaStream_t s, cudaLaunchAttribute* attr) {
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.stream = s;
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cfg;
+}
+
 // ---------------------------------------------------------------------------------------------
 // (a) r(i) = (prod_{k<=i} c_k) * (1 - c_{i+1}), i = 0..gamma-2 (Eq. 4);
 //     S = Top-K_i r(i) (Eq. 5).
@@ -17,6 +33,7 @@ __global__ void __launch_bounds__(32) select_prefixes_kernel(const float* __rest
                                                              double* __restrict__ r_out) {
     __shared__ double r_s[64];
     __shared__ int sel_s[64];
+    sb_pdl();
     const int b = blockIdx.x;
     const int lane = threadIdx.x;
     const int n = gamma - 1;
@@ -51,7 +68,9 @@ __global__ void __launch_bounds__(32) select_prefixes_kernel(const float* __rest
 int32_t launch_select(const float* conf, int B, int gamma, int K, int32_t* prefix_len, double* r_out,
                       cudaStream_t s) {
     if (B == 0) return D2SD_OK;
-    select_prefixes_kernel<<<B, 32, 0, s>>>(conf, gamma, K, prefix_len, r_out);
+    cudaLaunchAttribute attr[1];
+    cudaLaunchConfig_t cfg = sb_config(dim3(B), dim3(32), s, attr);
+    D2SD_CHECK_CUDA(cudaLaunchKernelEx(&cfg, select_prefixes_kernel, conf, gamma, K, prefix_len, r_out));
     D2SD_CHECK_LAUNCH("select_prefixes_kernel");
     return D2SD_OK;
 }
@@ -83,6 +102,7 @@ __global__ void build_tree_kernel(const int32_t* __restrict__ draft1, const int3
                                   int32_t* __restrict__ tree_len) {
     __shared__ int off_s[65];
     __shared__ int pre_s[64];
+    sb_pdl();
     const int b = blockIdx.x;
     if (threadIdx.x == 0) {
         int off = gamma;
@@ -136,8 +156,10 @@ int32_t launch_build_tree(const int32_t* draft1, const int32_t* draft2, const in
     int threads = ((T_cap + 31) / 32) * 32;
     if (threads > 256) threads = 256;
     if (threads < 32) threads = 32;
-    build_tree_kernel<<<B, threads, 0, s>>>(draft1, draft2, prefix_len, ctx_len, gamma, K, T_cap, W, tokens,
-                                            parent, depth, pos_id, branch_off, mask, tree_len);
+    cudaLaunchAttribute attr[1];
+    cudaLaunchConfig_t cfg = sb_config(dim3(B), dim3(threads), s, attr);
+    D2SD_CHECK_CUDA(cudaLaunchKernelEx(&cfg, build_tree_kernel, draft1, draft2, prefix_len, ctx_len, gamma, K, T_cap, W, tokens,
+                                       parent, depth, pos_id, branch_off, mask, tree_len));
     D2SD_CHECK_LAUNCH("build_tree_kernel");
     return D2SD_OK;
 }
@@ -156,6 +178,7 @@ __global__ void __launch_bounds__(32) select_third_kernel(const float* __restric
                                                           const int32_t* __restrict__ prefix_len, int gamma,
                                                           int32_t* __restrict__ third_len,
                                                           double* __restrict__ r3_out) {
+    sb_pdl();
     const int bk = blockIdx.x;  // b*K + k
     const int lane = threadIdx.x;
     const float* c = conf2 + (size_t)bk * gamma;
@@ -185,7 +208,9 @@ __global__ void __launch_bounds__(32) select_third_kernel(const float* __restric
 int32_t launch_select_third(const float* conf2, const int32_t* prefix_len, int B, int gamma, int K,
                             int32_t* third_len, double* r3_out, cudaStream_t s) {
     if (B == 0 || K == 0) return D2SD_OK;
-    select_third_kernel<<<B * K, 32, 0, s>>>(conf2, prefix_len, gamma, third_len, r3_out);
+    cudaLaunchAttribute attr[1];
+    cudaLaunchConfig_t cfg = sb_config(dim3(B * K), dim3(32), s, attr);
+    D2SD_CHECK_CUDA(cudaLaunchKernelEx(&cfg, select_third_kernel, conf2, prefix_len, gamma, third_len, r3_out));
     D2SD_CHECK_LAUNCH("select_third_kernel");
     return D2SD_OK;
 }
@@ -203,6 +228,7 @@ __global__ void build_tree3_kernel(const int32_t* __restrict__ draft1, const int
                                    uint32_t* __restrict__ mask, int32_t* __restrict__ tree_len) {
     __shared__ int off_s[129];   // [0..K) second level, [K..2K) third level, [2K] = end
     __shared__ int pre_s[64], thr_s[64];
+    sb_pdl();
     const int b = blockIdx.x;
     if (threadIdx.x == 0) {
         int off = gamma;
@@ -272,8 +298,10 @@ int32_t launch_build_tree3(const int32_t* draft1, const int32_t* draft2, const i
     int threads = ((T_cap + 31) / 32) * 32;
     if (threads > 256) threads = 256;
     if (threads < 32) threads = 32;
-    build_tree3_kernel<<<B, threads, 0, s>>>(draft1, draft2, draft3, prefix_len, third_len, ctx_len, gamma, K, T_cap,
-                                             W, tokens, parent, depth, pos_id, branch_off, mask, tree_len);
+    cudaLaunchAttribute attr[1];
+    cudaLaunchConfig_t cfg = sb_config(dim3(B), dim3(threads), s, attr);
+    D2SD_CHECK_CUDA(cudaLaunchKernelEx(&cfg, build_tree3_kernel, draft1, draft2, draft3, prefix_len, third_len, ctx_len, gamma, K,
+                                       T_cap, W, tokens, parent, depth, pos_id, branch_off, mask, tree_len));
     D2SD_CHECK_LAUNCH("build_tree3_kernel");
     return D2SD_OK;
 }
