@@ -235,8 +235,9 @@ class Workload:
 
         B, T, Hq, Hkv, d = cfg.B, cfg.T_cap, cfg.Hq, cfg.Hkv, cfg.d
         kv_rows = self.layers[0]["k_cache"].shape[0] * (cfg.page_size if cfg.paged else 1)
+        self.attn_impl = int(os.environ.get("D2SD_BENCH_ATTN_IMPL", "0"))  # kernel A/B runs only (d2sd.h: test knob)
         self.ws_attn = d2sd.cascade_workspace(B, T, Hq, Hkv, d, self.max_ctx, device=dev,
-                                              page_size=self.page_size, kv_rows=kv_rows)
+                                              page_size=self.page_size, kv_rows=kv_rows, impl=self.attn_impl)
         self.ws_acc = torch.empty(d2sd.accept_workspace_bytes(B, T, cfg.V), dtype=torch.uint8, device=dev)
         self.prefix_len = torch.empty((B, cfg.K), dtype=torch.int32, device=dev)
         self.tree = None
@@ -270,7 +271,7 @@ class Workload:
                                       self.kvmeta.get("kv_indices"), self.step_in["ctx_len"], L["tree_k"],
                                       L["tree_v"], t["mask"], t["tree_len"], self.max_ctx,
                                       page_size=self.page_size, phases=phases, out=self.outs[layer],
-                                      lse=self.lse, workspace=self.ws_attn)
+                                      lse=self.lse, workspace=self.ws_attn, impl=self.attn_impl)
 
     def accept(self):
         t = self.tree
@@ -290,7 +291,7 @@ class Workload:
     @staticmethod
     def attn_kernel_for(cfg) -> str:
         # api.cu: paged KV with more (request, kv head) pairs than one wave holds runs the two-tiles-per-CTA kernel
-        return "attn_cascade_tc_kernel" if cfg.paged and cfg.B * cfg.Hkv * 4 > 148 else "attn_stream_kernel"
+        return "attn_duo_kernel" if cfg.paged and cfg.B * cfg.Hkv * 4 > 148 else "attn_stream_kernel"
 
     @property
     def launches_per_step(self) -> int:

@@ -62,24 +62,89 @@ static int32_t make_plan(const d2sd_attn_params* p, AttnPlan* out) {
     pl.page_size = p->page_size;
     pl.max_ctx_len = p->max_ctx_len;
     pl.kv_rows = p->kv_rows;
-    pl.use_tc = false;
     pl.use_stream = false;
+    pl.use_duo = false;
     // auto: the one-tile-per-CTA kernel, except for paged KV with more (request, kv head) pairs than one wave holds:
     // there the two-tiles-per-CTA kernel amortises the 2 KiB page boxes over twice the query rows (config 5:
-    // 363 vs 416 us)
+    // 314 vs 416 us)
     const bool paged_multiwave = p->page_size > 0 && (int64_t)p->B * p->Hkv * 4 > sm_count();
-    if (p->impl == 3 || (p->impl == 0 && !paged_multiwave)) {
+    if (p->impl == 2 || (p->impl == 0 && paged_multiwave)) {
+        pl.use_duo = attn_duo_supported(pl);
+        D2SD_CHECK_SUPPORTED(pl.use_duo || p->impl != 2, "impl = 2 (two-tiles-per-CTA tcgen05 kernel) does not cover this shape");
+    }
+    if (!pl.use_duo && (p->impl == 3 || p->impl == 0)) {
         pl.use_stream = attn_stream_supported(pl);
         D2SD_CHECK_SUPPORTED(pl.use_stream || p->impl != 3, "impl = 3 (one-tile-per-CTA tcgen05 kernel) does not cover this shape");
-    }
-    if (!pl.use_stream && p->impl != 1 && p->impl != 3) {
-        pl.use_tc = attn_cascade_tc_supported(pl);
-        D2SD_CHECK_SUPPORTED(pl.use_tc || p->impl != 2, "impl = 2 (tcgen05) does not cover this shape");
     }
     const int rows = pl.T_cap * pl.G;
     const int max_ctx = p->max_ctx_len > 0 ? p->max_ctx_len : 1;
     int splits = p->num_splits;
-    if (pl.use_stream) {
+    if (pl.use_duo) {
+        // One CTA = (request, kv head, item, context chunk); an item is the M tiles (2i, 2i+1) or an odd last tile.
+        // A duo item costs two softmax sub-unit rounds per key tile, a solo item one: its chunks are about half
+        // as many.  One wave: chunk counts from the cost model; otherwise fixed chunks of 32 key tiles.
+        const int n_mt = ceil_div(rows, 128);
+        const int n_duo = n_mt / 2, odd = n_mt & 1;
+        const int max_tiles = ceil_div(p->max_ctx_len, 128) + ceil_div(pl.T_cap, 128);
+        const int64_t heads = (int64_t)pl.B * pl.Hkv;
+        const int budget = (int)(sm_count() / (heads > 0 ? heads : 1));
+        int ca = 1, cb = 1;
+        pl.tps_min = 1;
+        if (splits > 0) {
+            ca = splits;
+            cb = (splits + 1) / 2;
+        } else if (budget >= n_duo + odd) {
+            const double ua = 3600.0, ub = 1800.0, xa = 8000.0, xb = 5000.0;
+            auto cost = [&](int c, double u, double x) { return ceil_div(max_tiles, c) * u + (c > 1 ? x : 0.0); };
+            double best = 1e30;
+            const int ca_max = n_duo ? (budget - odd) / n_duo : 1;
+            for (int a2 = 1; a2 <= (n_duo ? ca_max : 1) && a2 <= 64; ++a2) {
+                int b_room = odd ? budget - n_duo * a2 : 0;
+                if (b_room > 64) b_room = 64;
+                double tb = 0.0;
+                int b_best = 1;
+                if (odd) {
+                    tb = 1e30;
+                    for (int b2 = 1; b2 <= b_room; ++b2) {
+                        const double t = cost(b2, ub, xb);
+                        if (t < tb) { tb = t; b_best = b2; }
+                    }
+                }
+                const double ta = n_duo ? cost(a2, ua, xa) : 0.0;
+                const double t = ta > tb ? ta : tb;
+                if (t < best) { best = t; ca = a2; cb = b_best; }
+            }
+        } else {
+            ca = ceil_div(max_tiles, 32);
+            cb = ceil_div(max_tiles, 64);
+            pl.tps_min = -1;  // fixed below
+        }
+        if (ca > 64) ca = 64;
+        if (cb > 64) cb = 64;
+        if (ca > max_tiles) ca = max_tiles;  // never an always-empty chunk
+        if (cb > max_tiles) cb = max_tiles;
+        if (ca < 1) ca = 1;
+        if (cb < 1) cb = 1;
+        pl.last_merges = pl.tps_min < 0 && splits == 0;
+        if (pl.tps_min < 0) pl.tps_min = ceil_div(max_tiles, n_duo ? ca : cb);
+        pl.n_mt = n_mt;
+        pl.n_pair = n_duo; pl.n_single = odd;
+        pl.chunks_a = ca;
+        pl.chunks_b = cb;
+        pl.chunk_keys = 0;
+        pl.num_splits = n_duo ? ca : cb;
+        pl.NS = 0;
+        pl.grp_rows = 256 * (ca > cb ? ca : cb);
+        const size_t n_groups = (size_t)pl.B * pl.Hkv * (n_duo + odd);
+        const size_t slot_rows = n_groups * pl.grp_rows;
+        D2SD_CHECK_SUPPORTED(n_groups * 2 * sizeof(unsigned) <= kWsHeaderBytes - 16, "B*Hkv*items = %zu groups > %zu",
+                             n_groups, (kWsHeaderBytes - 16) / (2 * sizeof(unsigned)));
+        pl.off_cnt = 0;
+        pl.cnt_bytes = kWsHeaderBytes;
+        pl.off_o = pl.cnt_bytes;
+        pl.off_lse = pl.off_o + align_up(slot_rows * pl.d * sizeof(float), 256);
+        pl.bytes = pl.off_lse + align_up(slot_rows * sizeof(float), 256);
+    } else if (pl.use_stream) {
         // One CTA = (request, kv head, M tile, context chunk).  M tiles (2p, 2p+1) over the same chunk form a
         // 2-CTA cluster that shares its key tiles; an odd last tile's chunks are paired without sharing.
         // One wave (enough SMs for every M tile of every (request, kv head)): the chunk counts are chosen
@@ -142,70 +207,6 @@ static int32_t make_plan(const d2sd_attn_params* p, AttnPlan* out) {
         const size_t slot_rows = n_groups * pl.grp_rows;
         D2SD_CHECK_SUPPORTED(n_groups * 2 * sizeof(unsigned) <= kWsHeaderBytes - 16, "B*Hkv*tiles = %zu groups > %zu",
                              n_groups, (kWsHeaderBytes - 16) / (2 * sizeof(unsigned)));
-        pl.off_cnt = 0;
-        pl.cnt_bytes = kWsHeaderBytes;
-        pl.off_o = pl.cnt_bytes;
-        pl.off_lse = pl.off_o + align_up(slot_rows * pl.d * sizeof(float), 256);
-        pl.bytes = pl.off_lse + align_up(slot_rows * sizeof(float), 256);
-    } else if (pl.use_tc) {
-        // Query tiles (2p, 2p+1) form pair items, an odd last tile the single item; every item gets its
-        // own run of context chunks (one CTA each).  A pair item does two units per key tile, a single
-        // item one, so the single item gets about half as many chunks.  With enough SMs for one wave the
-        // chunk counts fill the machine and every request cuts its own key tiles evenly (tps_min = 1);
-        // otherwise chunks have a fixed length and short requests simply use fewer of them.
-        const int n_mt = ceil_div(rows, 128);
-        pl.n_pair = n_mt / 2;
-        pl.n_single = n_mt & 1;
-        const int max_tiles = ceil_div(p->max_ctx_len, 128) + ceil_div(pl.T_cap, 128);
-        const int64_t heads = (int64_t)pl.B * pl.Hkv;
-        const int budget = (int)(sm_count() / (heads > 0 ? heads : 1));  // CTAs per (request, kv head), one wave
-        // Up to three query tiles in the one-wave regime: every tile is a split item (one query tile per
-        // CTA, the two key-parity states merged inside the CTA), which halves the partial-state exchange
-        // per CTA at the price of one more pass of the KV over the L2->SM crossbar (measured: config 2
-        // 22.3 -> 18.7 us, config 3 72.3 -> 69.1 us; with 8 query tiles, config 4, pairs stay ahead).
-        if (splits == 0 && budget >= n_mt && n_mt <= 3) { pl.n_pair = 0; pl.n_single = n_mt; }
-        int ca, cb;
-        pl.tps_min = 1;
-        if (splits > 0) {
-            ca = splits;
-            cb = (splits + 1) / 2;
-        } else if (budget >= pl.n_pair + pl.n_single) {
-            ca = cb = 1;
-            if (pl.n_pair > 0) {
-                // measured unit costs: a single item's units cost ~0.65 of a pair item's two (they are
-                // tensor-bound but fetch a whole K/V tile per unit), so cb : ca ~ 0.65
-                while (pl.n_pair * (ca + 1) + pl.n_single * ((13 * (ca + 1) + 10) / 20) <= budget) ++ca;
-                cb = (13 * ca + 10) / 20;
-                if (pl.n_single) cb = (budget - pl.n_pair * ca) / pl.n_single;
-            } else {
-                cb = budget / pl.n_single;
-            }
-        } else {
-            // more SMs' worth of (request, kv head) pairs than SMs: fixed chunks of ~32 key tiles (measured
-            // on config 5: 8 -> 467 us, 16 -> 379, 32 -> 363, 44 -> 359, 66 -> 413)
-            ca = ceil_div(max_tiles, 32);
-            cb = ceil_div(max_tiles, 64);
-            pl.tps_min = -1;  // fixed below
-        }
-        if (ca > 64) ca = 64;  // a group's CTAs wait for each other
-        if (cb > 64) cb = 64;
-        if (ca > max_tiles) ca = max_tiles;  // never an always-empty chunk
-        if (cb > max_tiles) cb = max_tiles;
-        if (ca < 1) ca = 1;
-        if (cb < 1) cb = 1;
-        if (pl.tps_min < 0) pl.tps_min = ceil_div(max_tiles, pl.n_pair ? ca : cb);
-        pl.chunks_a = ca;
-        pl.chunks_b = cb;
-        pl.chunk_keys = 0;
-        pl.num_splits = pl.n_pair ? ca : cb;
-        pl.NS = 0;
-        pl.grp_rows = 256 * (pl.n_pair ? (pl.n_single && cb > ca ? cb : ca) : cb);
-        const size_t n_groups = (size_t)pl.B * pl.Hkv * (pl.n_pair + pl.n_single);
-        const size_t slot_rows = n_groups * pl.grp_rows;
-        // The counter header has a FIXED size, so that one workspace can serve calls with different
-        // params one after another (the scratch of one call never lands on the counters of another).
-        D2SD_CHECK_SUPPORTED(n_groups * 2 * sizeof(unsigned) <= kWsHeaderBytes, "B*Hkv*items = %zu groups > %zu",
-                             n_groups, kWsHeaderBytes / (2 * sizeof(unsigned)));
         pl.off_cnt = 0;
         pl.cnt_bytes = kWsHeaderBytes;
         pl.off_o = pl.cnt_bytes;
@@ -319,7 +320,10 @@ int32_t d2sd_cascade_verify_attn(const d2sd_attn_params* p, const void* q, const
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     const int phases = p->phases ? p->phases : 7;
     const bool do_prefix = phases & 1, do_tree = phases & 2, do_merge = phases & 4;
-    if (pl.use_stream) {
+    if (pl.use_stream || pl.use_duo) {
+        auto launch_attn_stream = [&](const AttnPlan& pl_, const AttnArgs& a_, int mode_, float* dbg_, cudaStream_t s_) {
+            return pl_.use_duo ? launch_attn_duo(pl_, a_, mode_, dbg_, s_) : d2sd::launch_attn_stream(pl_, a_, mode_, dbg_, s_);
+        };
         a.counters = reinterpret_cast<unsigned*>(static_cast<char*>(workspace) + pl.off_cnt);
         if (dbg_state) {
             const size_t half = (size_t)pl.B * pl.T_cap * pl.Hq * (pl.d + 1);
@@ -329,19 +333,6 @@ int32_t d2sd_cascade_verify_attn(const d2sd_attn_params* p, const void* q, const
         const int mode = phases & 3;
         if (mode == 0) return D2SD_OK;
         return launch_attn_stream(pl, a, mode, nullptr, s);
-    }
-    if (pl.use_tc) {
-        // One fused launch: prefix tiles, tree tiles and the cascade merge.  phases selects which key
-        // tiles take part (1 = prefix only, 2 = tree only); dbg_state costs two extra launches.
-        a.counters = reinterpret_cast<unsigned*>(static_cast<char*>(workspace) + pl.off_cnt);
-        if (dbg_state) {
-            const size_t half = (size_t)pl.B * pl.T_cap * pl.Hq * (pl.d + 1);
-            if (int32_t st = launch_attn_cascade_tc(pl, a, 1, dbg_state, s)) return st;
-            if (int32_t st = launch_attn_cascade_tc(pl, a, 2, dbg_state + half, s)) return st;
-        }
-        const int mode = phases & 3;
-        if (mode == 0) return D2SD_OK;  // phases == 4: the merge is part of the launch
-        return launch_attn_cascade_tc(pl, a, mode, nullptr, s);
     }
     if (do_prefix || do_tree)
         if (int32_t st = launch_attn_mma(pl, a, do_prefix, do_tree, s)) return st;

@@ -1,5 +1,5 @@
 // Stage (c), generic path: split-KV flash attention on mma.sync (m16n8k16 bf16, fp32 accumulate).
-// Serves the shapes the fused tcgen05 kernel (attn_cascade_sm100.cu) does not cover -- GQA group sizes
+// Serves the shapes the fused tcgen05 kernels (attn_stream_sm100.cu, attn_duo_sm100.cu) do not cover -- GQA group sizes
 // that do not divide a 128-row query tile -- and impl = 1 (tests: an independent second CUDA path):
 // prefix chunks and the tree pass (<= T_cap keys under the ancestor mask) as one launch, merge as a
 // second.  Contiguous and paged KV.  PAPER.md:52, :124, :154.

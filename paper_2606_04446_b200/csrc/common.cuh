@@ -106,11 +106,10 @@ int32_t launch_commit_kv(const CommitArgs& a, cudaStream_t s);
 // Partial softmax states in the workspace.
 //  mma.sync path ("row layout"): O fp32 [B][NS][T_cap][Hq][d], LSE fp32 [B][NS][T_cap][Hq]; slots
 //    0..num_splits-1 are the prefix chunks, slot num_splits is the tree pass.
-//  tcgen05 path (attn_cascade_sm100.cu): a header of self-resetting group counters (zero between
-//    calls), then partials per group (request, kv head, item): O fp32 [group][grp_rows][d] and LSE
-//    fp32 [group][grp_rows]; a pair item holds chunk c's two query tiles at rows c*256.., a single
-//    item holds chunk c (its two key-parity states already merged) at rows c*128..; the tree keys are key tiles of
-//    the same kernel.
+//  tcgen05 kernels (attn_stream_sm100.cu, attn_duo_sm100.cu): a fixed 1 MiB header of self-resetting group
+//    counters (zero between calls) and the error word, then partials per group (request, kv head, M tile or
+//    item): O bf16 [group][grp_rows][d] and LSE fp32 [group][grp_rows]; chunk c of a group holds its rows at
+//    c*128.. (one tile per CTA) or c*256.. (two tiles per CTA); the tree keys are key tiles of the same kernel.
 struct AttnPlan {
     int B, T_cap, W, Hq, Hkv, G, d;
     float sm_scale;
@@ -120,16 +119,16 @@ struct AttnPlan {
     int num_splits;   // prefix chunks
     int chunk_keys;   // mma.sync path: keys per chunk (multiple of 64); tcgen05 cuts whole key tiles on device
     int NS;           // row layout: num_splits + 1
-    bool use_tc;      // tcgen05 prefix pass
-    // tcgen05: the query rows (T*G) of one kv head are cut into 128-row tiles; tiles (2p, 2p+1) form
-    // "pair item" p, an odd last tile is the "single item".  Item kinds get their own chunk counts.
+    // tcgen05: the query rows (T*G) of one kv head are cut into 128-row M tiles; tiles (2p, 2p+1) form a pair
+    // (a sharing cluster or a duo item), an odd last tile stands alone.  The kinds get their own chunk counts.
     int n_mt;                // 128-row query tiles per (request, kv head), from T_cap
     bool last_merges;        // several waves: the last CTA of a group to arrive merges it (nobody waits)
+    bool use_duo;            // the two-tiles-per-CTA sub-unit kernel (attn_duo_sm100.cu): n_pair duo items, n_single solo item
     bool use_stream;         // the one-tile-per-CTA kernel (attn_stream_sm100.cu): chunks_a per paired tile, chunks_b for an odd last tile
     int n_pair, n_single;    // items per (request, kv head), from T_cap
     int chunks_a, chunks_b;  // CTAs (context chunks) per pair item / per single item
     int tps_min;             // a chunk never holds fewer key tiles than this (unless the request ends)
-    int grp_rows;            // partial-state rows per group: max(chunks_a*256, chunks_b*256)
+    int grp_rows;            // partial-state rows per group: rows per chunk x max(chunks_a, chunks_b)
     size_t off_cnt, cnt_bytes, off_o, off_lse, bytes;
 };
 
@@ -148,9 +147,9 @@ int32_t launch_attn_mma(const AttnPlan& pl, const AttnArgs& a, bool do_prefix, b
                         cudaStream_t s);
 int32_t launch_attn_merge(const AttnPlan& pl, const AttnArgs& a, cudaStream_t s);
 // mode: bit 0 = prefix tiles, bit 1 = tree tiles; dbg_rows: fp32 [B][T_cap][Hq][d+1] instead of out/lse
-int32_t launch_attn_cascade_tc(const AttnPlan& pl, const AttnArgs& a, int mode, float* dbg_rows, cudaStream_t s);
-bool attn_cascade_tc_supported(const AttnPlan& pl);
 int32_t launch_attn_stream(const AttnPlan& pl, const AttnArgs& a, int mode, float* dbg_rows, cudaStream_t s);
 bool attn_stream_supported(const AttnPlan& pl);
+int32_t launch_attn_duo(const AttnPlan& pl, const AttnArgs& a, int mode, float* dbg_rows, cudaStream_t s);
+bool attn_duo_supported(const AttnPlan& pl);
 
 }  // namespace d2sd

@@ -243,12 +243,13 @@ def test_attn_batched_contiguous_ragged(d2sd, oracle, impl):
 
 
 def test_attn_tcgen05_is_the_default(d2sd):
-    """impl = 2 (force tcgen05) is accepted exactly where auto picks it: contiguous and 16-key-paged KV
-    with 128 % G == 0; a GQA group size that does not divide a query tile stays on mma.sync."""
+    """impl = 2, 3 (force a tcgen05 kernel) are accepted exactly where auto picks one: contiguous and 16-key-paged
+    KV with 128 % G == 0; a GQA group size that does not divide a query tile stays on mma.sync."""
     assert d2sd.cascade_workspace_bytes(1, 70, 32, 8, 128, 4096, kv_rows=4096, impl=2) > 0
     assert d2sd.cascade_workspace_bytes(1, 70, 32, 8, 128, 4096, page_size=16, kv_rows=8192, impl=2) > 0
-    with pytest.raises(d2sd.D2sdError):
-        d2sd.cascade_workspace_bytes(1, 70, 24, 8, 128, 4096, kv_rows=4096, impl=2)
+    for impl in (2, 3):
+        with pytest.raises(d2sd.D2sdError):
+            d2sd.cascade_workspace_bytes(1, 70, 24, 8, 128, 4096, kv_rows=4096, impl=impl)
 
 
 @pytest.mark.parametrize("impl", IMPLS)
