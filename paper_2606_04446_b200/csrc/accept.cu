@@ -83,20 +83,30 @@ vocab_scan_kernel(const __nv_bfloat16* __restrict__ logits, int64_t row_stride, 
     const __nv_bfloat16* rowp = logits + (size_t)row * row_stride;
     const int start = blockIdx.y * kScanChunk;
     const int end = min(V, start + kScanChunk);
-    float bv = -INFINITY, bs = 0.f;
-    int bi = INT_MAX;
     const int tid = threadIdx.x;
-    if ((reinterpret_cast<uintptr_t>(rowp) & 15) == 0) {
+    const bool aligned = (reinterpret_cast<uintptr_t>(rowp) & 15) == 0;
+    __shared__ __align__(128) uint4 stage[kScanChunk / 8];
+    __shared__ __align__(8) unsigned long long bars[2];
+    __shared__ float red_v[kScanThreads / 32], red_s[kScanThreads / 32];
+    __shared__ int red_i;
+    // Two passes over the thread's 64 values, both out of registers.  Pass 1 is the maximum alone, two bf16
+    // values per instruction (max.bf16x2 returns the other operand for a NaN, so NaNs drop out); the block
+    // agrees on it; pass 2 -- only in the threads that hold the maximum -- finds its first index.  The index
+    // bookkeeping of a one-pass argmax (two compares and two selects per value) made the scan ALU-bound.
+    uint4 x[kVec];
+    int nvec = 0;
+    float xt = -INFINITY;  // this thread's element of the < 8 values behind the last whole vector
+    float m = -INFINITY;
+    if (aligned) {
         // The chunk is staged through shared memory by two bulk copies (one elected thread, mbarrier
         // completion): 32 KiB per CTA are in flight whatever the compiler does with the consuming loop
         // (ptxas interleaves plain vector loads with their compares and keeps only two in flight).
-        const int nvec = (end - start) >> 3;
-        __shared__ __align__(128) uint4 stage[kScanChunk / 8];
-        __shared__ __align__(8) unsigned long long bars[2];
+        nvec = (end - start) >> 3;
         const uint32_t bar0 = (uint32_t)__cvta_generic_to_shared(bars);
         const uint32_t st0 = (uint32_t)__cvta_generic_to_shared(stage);
         const int nv0 = min(nvec, kScanChunk / 16), nv1 = nvec - nv0;  // first / second half
         if (tid == 0) {
+            red_i = INT_MAX;
             asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar0));
             asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar0 + 8));
             asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -115,68 +125,91 @@ vocab_scan_kernel(const __nv_bfloat16* __restrict__ logits, int64_t row_stride, 
                     "l"(0x12F0000000000000ull) : "memory");
             }
         }
+        const int tail0 = start + nvec * 8;
+        if (tail0 + tid < end) xt = __bfloat162float(rowp[tail0 + tid]);
         __syncthreads();  // barrier initialisation visible to the waiting threads
-        uint4 x[kVec];
 #pragma unroll
         for (int u = 0; u < kVec; ++u) {
             if (u == 0 && nv0 > 0) scan_mbar_wait(bar0);
             if (u == kVec / 2 && nv1 > 0) scan_mbar_wait(bar0 + 8);
-            const int v = tid + u * kScanThreads;
+            const int v = tid + u * kScanThreads;  // absent vectors hold -inf
             x[u] = v < nvec ? stage[v] : make_uint4(0xFF80FF80u, 0xFF80FF80u, 0xFF80FF80u, 0xFF80FF80u);
         }
+        uint32_t m2[4] = {0xFF80FF80u, 0xFF80FF80u, 0xFF80FF80u, 0xFF80FF80u};
 #pragma unroll
         for (int u = 0; u < kVec; ++u) {
-            const int idx = start + (tid + u * kScanThreads) * 8;  // absent vectors hold -inf: never win
-            arg_update_word(x[u].x, idx, bv, bi);
-            arg_update_word(x[u].y, idx + 2, bv, bi);
-            arg_update_word(x[u].z, idx + 4, bv, bi);
-            arg_update_word(x[u].w, idx + 6, bv, bi);
+            asm("max.bf16x2 %0, %0, %1;" : "+r"(m2[0]) : "r"(x[u].x));
+            asm("max.bf16x2 %0, %0, %1;" : "+r"(m2[1]) : "r"(x[u].y));
+            asm("max.bf16x2 %0, %0, %1;" : "+r"(m2[2]) : "r"(x[u].z));
+            asm("max.bf16x2 %0, %0, %1;" : "+r"(m2[3]) : "r"(x[u].w));
         }
-        const int tail0 = start + nvec * 8;  // < 8 leftover elements of the chunk
-        float xt = -INFINITY;
-        if (tail0 + tid < end) {
-            xt = __bfloat162float(rowp[tail0 + tid]);
-            arg_update(xt, tail0 + tid, bv, bi);
+        asm("max.bf16x2 %0, %0, %1;" : "+r"(m2[0]) : "r"(m2[1]));
+        asm("max.bf16x2 %0, %0, %1;" : "+r"(m2[2]) : "r"(m2[3]));
+        asm("max.bf16x2 %0, %0, %1;" : "+r"(m2[0]) : "r"(m2[2]));
+        m = fmaxf(fmaxf(bf_lo(m2[0]), bf_hi(m2[0])), xt);  // fmaxf drops a NaN as well
+    } else {  // misaligned row start (odd strides): plain loads
+        if (tid == 0) red_i = INT_MAX;
+        for (int i = start + tid; i < end; i += kScanThreads) m = fmaxf(m, __bfloat162float(rowp[i]));
+        __syncthreads();
+    }
+    // the block's maximum
+    float mb = m;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) mb = fmaxf(mb, __shfl_xor_sync(0xffffffffu, mb, o));
+    if ((tid & 31) == 0) red_v[tid >> 5] = mb;
+    __syncthreads();
+    mb = red_v[0];
+#pragma unroll
+    for (int w = 1; w < kScanThreads / 32; ++w) mb = fmaxf(mb, red_v[w]);
+    // its first index (IEEE equality: -0 == +0, a NaN never matches), and the sum of e^(x - max)
+    float bs = 0.f;
+    if (aligned) {
+        if (m == mb) {
+            int cand = INT_MAX;
+#pragma unroll
+            for (int u = 0; u < kVec; ++u) {  // (unrolled: x stays in registers)
+                const int v = tid + u * kScanThreads;
+                if (cand != INT_MAX || v >= nvec) continue;
+                const uint32_t w[4] = {x[u].x, x[u].y, x[u].z, x[u].w};
+#pragma unroll
+                for (int e = 3; e >= 0; --e) {
+                    if (bf_hi(w[e]) == mb) cand = start + v * 8 + 2 * e + 1;
+                    if (bf_lo(w[e]) == mb) cand = start + v * 8 + 2 * e;
+                }
+            }
+            if (cand == INT_MAX && xt == mb) cand = start + nvec * 8 + tid;
+            if (cand != INT_MAX) atomicMin(&red_i, cand);
         }
-        if (kSum && bv > -INFINITY) {
+        if (kSum && mb > -INFINITY) {
 #pragma unroll
             for (int u = 0; u < kVec; ++u) {
                 const uint32_t w[4] = {x[u].x, x[u].y, x[u].z, x[u].w};
 #pragma unroll
-                for (int e = 0; e < 4; ++e) bs += __expf(bf_lo(w[e]) - bv) + __expf(bf_hi(w[e]) - bv);
+                for (int e = 0; e < 4; ++e) bs += __expf(bf_lo(w[e]) - mb) + __expf(bf_hi(w[e]) - mb);
             }
-            bs += __expf(xt - bv);
+            bs += __expf(xt - mb);
         }
-    } else {  // misaligned row start (odd strides): plain loads
-        for (int i = start + tid; i < end; i += kScanThreads) arg_update(__bfloat162float(rowp[i]), i, bv, bi);
-        if (kSum && bv > -INFINITY)
-            for (int i = start + tid; i < end; i += kScanThreads) bs += __expf(__bfloat162float(rowp[i]) - bv);
+    } else {
+        if (m == mb) {
+            for (int i = start + tid; i < end; i += kScanThreads)
+                if (__bfloat162float(rowp[i]) == mb) {
+                    atomicMin(&red_i, i);
+                    break;
+                }
+        }
+        if (kSum && mb > -INFINITY)
+            for (int i = start + tid; i < end; i += kScanThreads) bs += __expf(__bfloat162float(rowp[i]) - mb);
     }
+    if (kSum) {
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        const float ov = __shfl_xor_sync(0xffffffffu, bv, o);
-        const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
-        if (kSum) {
-            const float os = __shfl_xor_sync(0xffffffffu, bs, o);
-            state_merge(ov, oi, os, bv, bi, bs);
-        } else {
-            arg_update(ov, oi, bv, bi);
-        }
-    }
-    __shared__ float sv[kScanThreads / 32], ss[kScanThreads / 32];
-    __shared__ int si[kScanThreads / 32];
-    if ((tid & 31) == 0) {
-        sv[tid >> 5] = bv;
-        si[tid >> 5] = bi;
-        ss[tid >> 5] = bs;
+        for (int o = 16; o > 0; o >>= 1) bs += __shfl_xor_sync(0xffffffffu, bs, o);
+        if ((tid & 31) == 0) red_s[tid >> 5] = bs;
     }
     __syncthreads();
     if (tid == 0) {
-        for (int w = 1; w < kScanThreads / 32; ++w) {
-            if (kSum) state_merge(sv[w], si[w], ss[w], bv, bi, bs);
-            else arg_update(sv[w], si[w], bv, bi);
-        }
-        part[(size_t)row * n_chunks + blockIdx.y] = ScanPart{bv, bi, bs, 0.f};
+        if (kSum)
+            for (int w = 1; w < kScanThreads / 32; ++w) bs += red_s[w];
+        part[(size_t)row * n_chunks + blockIdx.y] = ScanPart{mb, red_i, bs, 0.f};
     }
 }
 
