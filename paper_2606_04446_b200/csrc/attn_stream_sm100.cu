@@ -95,10 +95,6 @@ static_assert((kNumBars + 1) * 8 <= 512, "barrier area");
 static_assert(kSmemUsed + 512 <= kSmemBytes, "shared memory budget");  // the kernel checks the actual alignment slack
 
 // ---- cluster (2-CTA sharing pair) ---------------------------------------------------------------
-__device__ __forceinline__ void cluster_sync_all() {  // every thread of both CTAs
-    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
-    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
-}
 // tcgen05.commit that arrives on the barrier at the same offset in every CTA of `mask`
 __device__ __forceinline__ void tc_commit_mc(uint32_t bar, uint16_t mask) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(bar),
@@ -540,9 +536,15 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
             }
         }
       }
+      // The pair's last barrier, arrival half: this warp has issued everything it will ever send to the peer (multicast
+      // loads, multicast commits).  The wait half sits at the kernel's end, an epilogue later, and costs nothing there.
+      __syncwarp();
+      if (pair) asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
     } else {
       asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegsSoftmax));
-      if (!idle) {
+      if (idle) {
+        if (pair) asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+      } else {
         // ===== softmax: team t (warps 4t..4t+3) owns the sub-units n = t (mod 4); thread (w, lane) owns query
         // row w*32 + lane (TMEM lane) and the sub-unit's 64 scores.  Four warps per scheduler work on four
         // different sub-units: while one is in its exponentials the others load, take maxima, pack, store. =====
@@ -702,6 +704,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
         const int t_last = (n_sub - 1) & 3;
         if (warp_active && n_sub > 0 && t_last == t) xm[t * kTileM + rl] = m_mine;  // owner of the last sub-unit
         mbar_wait(bar(kBarAllDone), 0);  // every MMA done: O is final, the rings are free
+        if (pair) asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");  // (see the control warps)
         //@T 56
         named_bar_sync(9, 512);
         const float m_fin = n_sub > 0 ? xm[t_last * kTileM + rl] : -INFINITY;
@@ -818,7 +821,8 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
             } else {
                 int ok = 1;
                 if (warp == 0 && lane == 0) {
-                    __threadfence();
+                    // (release at gpu scope, cumulative over the other threads' writes ordered before it by the
+                    // barrier above: no separate fence)
                     asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(cnt) : "memory");
                     unsigned seen, spins = 0;
                     do {
@@ -861,7 +865,9 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(kTmemCols) : "memory");
     }
     //@T 61
-    if (pair) cluster_sync_all();  // no CTA leaves while its peer may still signal its barriers
+    // no CTA leaves while its peer may still signal its barriers (every thread of the pair arrived after its last
+    // remote operation; by now the peer's arrivals are an epilogue old)
+    if (pair) asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
     //@T 62
 }
 
