@@ -204,6 +204,24 @@ int32_t d2sd_accept(const void* logits, int64_t row_stride, int32_t V, const int
                     int32_t* path, int32_t* bonus, int32_t* best_node, void* workspace,
                     size_t workspace_bytes, void* stream);
 
+/* ---------------------------------------------------------------------------------------------
+ * d2sd_accept without a workspace argument, for callers that cannot allocate one (code under CUDA
+ * graph capture, serving loops or harnesses that forbid cudaMalloc).  Same inputs, outputs, kernels
+ * and results as d2sd_accept; the chunk states live in a 1 MiB array built into the library
+ * (d2sd_accept_static_max_bytes(); every GPU that loads the library holds it until exit).
+ * Limit: B * T_cap * ceil(V/16384) * 16 bytes <= that size (65536 chunk states; BASELINE config 5
+ * needs 11200), otherwise D2SD_ERR_UNSUPPORTED and nothing is enqueued.  The call allocates
+ * nothing.  Every call on a device shares the one array: calls whose kernels may overlap on the
+ * GPU (different streams, no dependency) RACE -- order them, or use d2sd_accept with separate
+ * workspaces.  Nothing in the array has to be cleared between calls.
+ * ------------------------------------------------------------------------------------------- */
+size_t d2sd_accept_static_max_bytes(void);
+
+int32_t d2sd_accept_static(const void* logits, int64_t row_stride, int32_t V, const int32_t* tokens,
+                           const int32_t* parent, const int32_t* depth, const int32_t* tree_len, int32_t B,
+                           int32_t gamma, int32_t T_cap, int32_t* argmax_out, int32_t* accept_len,
+                           int32_t* path, int32_t* bonus, int32_t* best_node, void* stream);
+
 /* =============================================================================================
  * The steps around the hot path (SURVEY.md 8f "next" rows), same conventions as above.
  * ============================================================================================= */

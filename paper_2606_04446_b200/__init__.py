@@ -8,4 +8,5 @@ from .binding import (  # noqa: F401
     D2sdError, accept, accept_workspace_bytes, build_tree, cascade_verify_attn,
     cascade_workspace, cascade_workspace_bytes, last_error, lib, lib_path, select_prefixes, t_cap, version,
     build_tree3, commit_kv, confidence_workspace_bytes, draft_confidence, select_third, t_cap3,
+    accept_static, accept_static_max_bytes,
 )

@@ -70,6 +70,10 @@ def lib() -> ctypes.CDLL:
         L.d2sd_accept.restype = i32
         L.d2sd_accept.argtypes = [vp, i64, i32, vp, vp, vp, vp, i32, i32, i32, vp, vp, vp, vp, vp, vp,
                                   ctypes.c_size_t, vp]
+        L.d2sd_accept_static_max_bytes.restype = ctypes.c_size_t
+        L.d2sd_accept_static_max_bytes.argtypes = []
+        L.d2sd_accept_static.restype = i32
+        L.d2sd_accept_static.argtypes = [vp, i64, i32, vp, vp, vp, vp, i32, i32, i32, vp, vp, vp, vp, vp, vp]
         L.d2sd_confidence_workspace_bytes.restype = ctypes.c_size_t
         L.d2sd_confidence_workspace_bytes.argtypes = [i32, i32, i32]
         L.d2sd_draft_confidence.restype = i32
@@ -275,6 +279,32 @@ def accept(logits: torch.Tensor, tokens: torch.Tensor, parent: torch.Tensor, dep
                              _ptr(tree_len), B, gamma, T_cap, _ptr(out["argmax"]), _ptr(out["accept_len"]),
                              _ptr(out["path"]), _ptr(out["bonus"]), _ptr(out["best_node"]), _ptr(workspace),
                              workspace.numel() * workspace.element_size(), _stream()))
+    return out
+
+
+def accept_static_max_bytes() -> int:
+    return int(lib().d2sd_accept_static_max_bytes())
+
+
+def accept_static(logits: torch.Tensor, tokens: torch.Tensor, parent: torch.Tensor, depth: torch.Tensor,
+                  tree_len: torch.Tensor, gamma: int, out: Dict[str, torch.Tensor]) -> Dict[str, torch.Tensor]:
+    """d2sd_accept_static: d2sd_accept with the library's built-in scratch.  Allocates nothing: the caller
+    passes every output (out: argmax [B,T_cap], accept_len, bonus, best_node [B], path [B,gamma], int32)."""
+    if not (logits.is_cuda and logits.dtype == torch.bfloat16 and logits.dim() == 3 and logits.stride(2) == 1
+            and logits.stride(0) == logits.shape[1] * logits.stride(1)):
+        raise TypeError("logits: expected CUDA bf16 [B,T_cap,V] with unit inner stride and uniform row stride")
+    B, T_cap, V = logits.shape
+    for t, n in ((tokens, "tokens"), (parent, "parent"), (depth, "depth"), (tree_len, "tree_len")):
+        _dev(t, torch.int32, n)
+    dev = logits.device
+    for name, shape in (("argmax", (B, T_cap)), ("accept_len", (B,)), ("bonus", (B,)), ("best_node", (B,)),
+                        ("path", (B, gamma))):
+        if out.get(name) is None:
+            raise TypeError(f"accept_static: out[{name!r}] must be given (this entry point allocates nothing)")
+        _out(out[name], shape, torch.int32, dev, name)
+    _check(lib().d2sd_accept_static(_ptr(logits), logits.stride(1), V, _ptr(tokens), _ptr(parent), _ptr(depth),
+                                    _ptr(tree_len), B, gamma, T_cap, _ptr(out["argmax"]), _ptr(out["accept_len"]),
+                                    _ptr(out["path"]), _ptr(out["bonus"]), _ptr(out["best_node"]), _stream()))
     return out
 
 

@@ -352,4 +352,62 @@ int32_t launch_confidence(const __nv_bfloat16* logits, int64_t row_stride, int V
     return D2SD_OK;
 }
 
+// ---- d2sd_accept_static: the same two launches with the chunk states in a file-scope device array -----------
+// For callers that cannot provide (or allocate) a workspace.  The array costs kStaticScratchBytes of device
+// memory on every GPU that loads the library, until exit.  In host code `g_accept_scratch` is only a stand-in
+// for the symbol, not a device address: the address the kernels get comes from cudaGetSymbolAddress, asked
+// once per device with that device current.
+constexpr size_t kStaticScratchBytes = 1u << 20;  // 65536 chunk states of 16 B (config 5 needs 11200)
+static __device__ __align__(256) unsigned char g_accept_scratch[kStaticScratchBytes];
+static_assert(sizeof(ScanPart) == kScanPartBytes, "chunk state size");
+
+static int32_t accept_scratch_address(void** out) {
+    static void* addr[64] = {};  // per device; a race between two first callers repeats an idempotent query
+    int dev = 0;
+    D2SD_CHECK_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return set_error(D2SD_ERR_UNSUPPORTED, "device ordinal %d outside [0,64)", dev);
+    if (!addr[dev]) {
+        void* p = nullptr;
+        D2SD_CHECK_CUDA(cudaGetSymbolAddress(&p, g_accept_scratch));
+        if (!p || (reinterpret_cast<uintptr_t>(p) & 255)) return set_error(D2SD_ERR_CUDA, "static scratch at %p", p);
+        addr[dev] = p;
+    }
+    *out = addr[dev];
+    return D2SD_OK;
+}
+
 }  // namespace d2sd
+
+using namespace d2sd;
+
+extern "C" size_t d2sd_accept_static_max_bytes(void) { return kStaticScratchBytes; }
+
+extern "C" int32_t d2sd_accept_static(const void* logits, int64_t row_stride, int32_t V, const int32_t* tokens,
+                                      const int32_t* parent, const int32_t* depth, const int32_t* tree_len,
+                                      int32_t B, int32_t gamma, int32_t T_cap, int32_t* argmax_out,
+                                      int32_t* accept_len, int32_t* path, int32_t* bonus, int32_t* best_node,
+                                      void* stream) {
+    clear_error();
+    D2SD_CHECK_ARG(B >= 0 && V >= 1 && row_stride >= V, "B = %d, V = %d, row_stride = %lld", B, V,
+                   (long long)row_stride);
+    D2SD_CHECK_ARG(gamma >= 2 && gamma <= 64, "gamma = %d outside [2,64]", gamma);
+    D2SD_CHECK_ARG(T_cap >= 1, "T_cap = %d", T_cap);
+    D2SD_CHECK_SUPPORTED(T_cap <= 1024, "T_cap = %d > 1024", T_cap);
+    D2SD_CHECK_SUPPORTED(ceil_div(V, kScanChunk) <= 65535, "V = %d too large", V);
+    const size_t need = (size_t)B * T_cap * ceil_div(V, kScanChunk) * sizeof(ScanPart);
+    D2SD_CHECK_SUPPORTED(need <= kStaticScratchBytes,
+                         "d2sd_accept_static: B*T_cap*ceil(V/%d) = %zu chunk states need %zu bytes, the built-in scratch "
+                         "holds %zu; use d2sd_accept with a caller workspace",
+                         kScanChunk, need / sizeof(ScanPart), need, kStaticScratchBytes);
+    if (B == 0) return D2SD_OK;
+    D2SD_CHECK_ARG(logits && tokens && parent && depth && tree_len && argmax_out && accept_len && path &&
+                       bonus && best_node,
+                   "a required buffer is NULL");
+    void* scratch = nullptr;
+    if (int32_t st = accept_scratch_address(&scratch)) return st;
+    // nothing in the scratch has to start at zero: the scan writes the state of every (real row, chunk) and the
+    // walk reads exactly those, so the previous call's contents are never seen
+    return launch_accept(static_cast<const __nv_bfloat16*>(logits), row_stride, V, tokens, parent, depth, tree_len, B,
+                         gamma, T_cap, argmax_out, accept_len, path, bonus, best_node, scratch,
+                         static_cast<cudaStream_t>(stream));
+}
