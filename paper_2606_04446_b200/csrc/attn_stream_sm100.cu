@@ -84,8 +84,8 @@ enum : uint32_t {
     kBarSFull = kBarVEmpty + kRingV,     // [4] Q.K^T of a sub-unit has completed
     kBarSFree = kBarSFull + kTeams,      // [4] the owning team has read S into registers
     kBarPFull = kBarSFree + kTeams,      // [4] the owning team has written P
-    kBarPFree = kBarPFull + kTeams,      // [4] P.V of a sub-unit has completed (P buffer reusable, O current)
-    kBarRef = kBarPFree + kTeams,        // [4 teams][4 warps] the team's warp has published its rows' reference maxima
+    kBarPFree = kBarPFull + kTeams,      // [8] P.V of sub-unit n has completed: barrier n & 7 (P buffer reusable, O current)
+    kBarRef = kBarPFree + 8,             // [4 teams][4 warps] the team's warp has published its rows' reference maxima
     kBarVFix = kBarRef + 4 * kTeams,     // [2] V rows behind a ragged tile end are zero (<= 2 ragged tiles per CTA)
     kBarAllDone = kBarVFix + 2,
     kNumBars = kBarAllDone + 1,
@@ -290,6 +290,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
             mbar_init(bar(kBarSFree + t), 4);  // one elected arrival per warp of the owning team
             mbar_init(bar(kBarPFull + t), 4);
             mbar_init(bar(kBarPFree + t), 1);
+            mbar_init(bar(kBarPFree + 4 + t), 1);
             for (int w = 0; w < 4; ++w) mbar_init(bar(kBarRef + 4 * t + w), 1);
         }
         mbar_init(bar(kBarVFix + 0), 1);
@@ -527,7 +528,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
                     for (int ks = 0; ks < kSubN / 16; ++ks)
                         if (ks < ksteps)
                             umma_ts(od, pd + ks * 8, vd + (uint64_t)((pc.hf * (kSubN / 16) + ks) * (2048 >> 4)), kIdescPV, (pc.n > 0) | ks);
-                    tc_commit(bar(kBarPFree + t));
+                    tc_commit(bar(kBarPFree + (pc.n & 7)));
                     if (cur_last_half(pc)) release(bar(kBarVEmpty + vi));  // V is free once the tile's last P.V has completed
                     //@T (pc.n < 8 ? 17 + 2 * pc.n : 63)
                     cur_next(pc);
@@ -578,7 +579,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
                 if (!warp_active) {  // a warp without rows only keeps the barrier phases in step
                     if (lane == 0) {
                         mbar_arrive(bar(kBarSFree + t));
-                        if (n >= kTeams) mbar_wait(bar(kBarPFree + t), par ^ 1);
+                        if (n >= kTeams) mbar_wait(bar(kBarPFree + ((n - 4) & 7)), ((n - 4) >> 3) & 1);
                         mbar_arrive(bar(kBarPFull + t));
                     }
                     __syncwarp();
@@ -639,11 +640,11 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
                 if (__any_sync(0xffffffffu, need)) {
                     // O holds sub-units < n relative to m_prev: wait for P.V of sub-unit n-1, rescale this row.
                     // P.V of sub-unit n cannot start before this thread releases P_n below.
-                    // A parity wait is only sound for the current or the preceding phase.  This thread last observed
-                    // this barrier (if at all) several phases ago, but its own P guard at sub-unit n-4 has seen P.V of
-                    // n-8 complete, hence also n-9: waiting for n-5 and then n-1 walks the phases one by one.
-                    if (n - 1 >= kTeams) mbar_wait(bar(kBarPFree + tp), (((n - 1) >> 2) & 1) ^ 1);
-                    mbar_wait(bar(kBarPFree + tp), ((n - 1) >> 2) & 1);
+                    // A parity wait is only sound when the barrier's preceding phase is known to be complete and its
+                    // next one cannot be: P.V completions are spread over eight barriers (sub-unit n -> barrier n & 7,
+                    // a phase every eight sub-units).  For barrier (n-1) & 7: this thread's own P guard at sub-unit n-4
+                    // has seen P.V of n-8 complete, hence n-9 (the P.V stream is in order); P.V of n+7 needs P_n.
+                    mbar_wait(bar(kBarPFree + ((n - 1) & 7)), ((n - 1) >> 3) & 1);
                     tc_fence_after();
                     const float alpha = need ? (m_prev == -INFINITY ? 0.f : ex2((m_prev - m_new) * c2)) : 1.f;
 #pragma unroll 1
@@ -662,8 +663,9 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
                     tmem_wait_st();
                     tc_fence_before();
                 }
-                // the P buffer is free once P.V of sub-unit n-4 has completed
-                if (n >= kTeams) mbar_wait(bar(kBarPFree + t), par ^ 1);
+                // the P buffer is free once P.V of sub-unit n-4 has completed (this team sees barriers t and t+4 in
+                // alternation, each phase after phase)
+                if (n >= kTeams) mbar_wait(bar(kBarPFree + ((n - 4) & 7)), ((n - 4) >> 3) & 1);
                 // a row with every key so far masked has m_ref = -inf: exp2(-inf - 0) = 0, not NaN
                 const float ms = m_new == -INFINITY ? 0.f : m_new * c2;
                 float sum0 = 0.f, sum1 = 0.f;
