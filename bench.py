@@ -236,8 +236,10 @@ class Workload:
         B, T, Hq, Hkv, d = cfg.B, cfg.T_cap, cfg.Hq, cfg.Hkv, cfg.d
         kv_rows = self.layers[0]["k_cache"].shape[0] * (cfg.page_size if cfg.paged else 1)
         self.attn_impl = int(os.environ.get("D2SD_BENCH_ATTN_IMPL", "0"))  # kernel A/B runs only (d2sd.h: test knob)
+        self.attn_splits = int(os.environ.get("D2SD_BENCH_ATTN_SPLITS", "0"))  # chunk-count sweeps only (d2sd.h: test knob)
         self.ws_attn = d2sd.cascade_workspace(B, T, Hq, Hkv, d, self.max_ctx, device=dev,
-                                              page_size=self.page_size, kv_rows=kv_rows, impl=self.attn_impl)
+                                              page_size=self.page_size, kv_rows=kv_rows, impl=self.attn_impl,
+                                              num_splits=self.attn_splits)
         self.ws_acc = torch.empty(d2sd.accept_workspace_bytes(B, T, cfg.V), dtype=torch.uint8, device=dev)
         self.prefix_len = torch.empty((B, cfg.K), dtype=torch.int32, device=dev)
         self.tree = None
@@ -271,7 +273,8 @@ class Workload:
                                       self.kvmeta.get("kv_indices"), self.step_in["ctx_len"], L["tree_k"],
                                       L["tree_v"], t["mask"], t["tree_len"], self.max_ctx,
                                       page_size=self.page_size, phases=phases, out=self.outs[layer],
-                                      lse=self.lse, workspace=self.ws_attn, impl=self.attn_impl)
+                                      lse=self.lse, workspace=self.ws_attn, impl=self.attn_impl,
+                                      num_splits=self.attn_splits)
 
     def accept(self):
         t = self.tree

@@ -118,7 +118,9 @@ typedef struct d2sd_attn_params {
     int32_t max_ctx_len; /* host-side upper bound on ctx_len[b]; sizes the split-KV grid         */
     int64_t kv_rows;     /* token rows in k_cache/v_cache: contiguous: >= kv_indptr[B] (sum L_b);
                             paged: num_pages * page_size.  Bounds the TMA tensor maps.           */
-    int32_t num_splits;  /* TEST KNOB, leave 0: key chunks per (request, kv head) chosen from the shape (<= 64) */
+    int32_t num_splits;  /* TEST KNOB, leave 0: key chunks per (request, kv head) chosen from the shape (<= 64);
+                            one-tile-per-CTA kernel: values >= 256 mean (chunks of an odd last tile << 8) |
+                            chunks of a paired tile                                                        */
     int32_t impl;        /* TEST KNOB, leave 0 (auto).  1 = force the mma.sync kernels; 2 = force the fused
                             two-query-tiles-per-CTA tcgen05 kernel; 3 = force the fused one-query-tile-per-
                             CTA tcgen05 kernel (2, 3: D2SD_ERR_UNSUPPORTED if the shape is outside them)  */

@@ -158,7 +158,10 @@ static int32_t make_plan(const d2sd_attn_params* p, AttnPlan* out) {
         const int budget = (int)((sm_count() & ~1) / (heads > 0 ? heads : 1));
         int ca = 1, cb = 1;
         pl.tps_min = 1;
-        if (splits > 0) {
+        if (splits >= 256) {  // test knob: (chunks_b << 8) | chunks_a
+            ca = splits & 255;
+            cb = splits >> 8;
+        } else if (splits > 0) {
             ca = cb = splits;
         } else if (budget >= 2 * n_pairs + 2 * odd) {
             const int rows_last = rows - (n_mt - 1) * 128;

@@ -268,7 +268,6 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
     auto bar = [&](uint32_t i) { return bar0 + 8u * i; };
     volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(smem_gen + kOffBar + 8u * kTmemSlot);
 
-    //@T 0
     // static part of the work decode (no global memory): which cluster kind this CTA belongs to
     const int n_pairs = pl.n_mt >> 1;
     const int pair_ctas = n_pairs * 2 * pl.chunks_a;
@@ -410,16 +409,17 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
         }
         int page_cur = page_of(0);
         int n_ragged = 0;
+        int i = 0;            // ring slot of tile jj
+        uint32_t round = 0;   // parity of jj / ring
         for (int jj = 0; jj < wk.n_tiles; ++jj) {
             const TileInfo ti = tile_info(jj);
             const int page_next = page_of(jj + 1);
-            const int i = jj % ring;
             const uint32_t dst = smem + ring_off + i * kKvTileBytes;
             const uint32_t fb = bar(bar_full + i);
             const bool by_page = paged && !ti.tree;
             const int n_pages = (ti.valid + 15) >> 4;
             if (lane == 0) {
-                mbar_wait(bar(bar_empty + i), ((jj / ring) & 1) ^ 1);
+                mbar_wait(bar(bar_empty + i), round ^ 1u);
                 mbar_expect_tx(fb, by_page ? (uint32_t)n_pages * 4096u : kKvTileBytes);
             }
             __syncwarp();
@@ -441,7 +441,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
             }
             //@T (jj < 6 ? 8 + jj : 63)
             if (is_v && (ti.valid & 15) != 0) {
-                mbar_wait(fb, (jj / ring) & 1);  // this fill has landed (every lane observes it)
+                mbar_wait_warp(lane, fb, round);  // this fill has landed (every lane observes it)
                 const int n_rows = ((ti.valid + 15) & ~15) - ti.valid;
                 for (int e = lane; e < n_rows * 16; e += 32) {  // 16 x 16 B per row
                     const int row = ti.valid + (e >> 4), c16 = e & 15;
@@ -456,6 +456,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
             }
             __syncwarp();
             page_cur = page_next;
+            if (++i == ring) { i = 0; round ^= 1u; }
         }
       } else if (warp == 18 || warp == 19) {
         // ===== MMA issuers (warp 18: Q.K^T stream, warp 19: P.V stream): one elected thread each walks the sub-unit sequence (two 64-key halves per key tile, a
@@ -471,67 +472,85 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
                 if (wk.share) tc_commit_mc(b, 3);
                 else { tc_commit(b); if (pair) tc_commit(b); }  // a pair cluster's barriers count two releases
             };
-            // cursor over the sub-unit sequence: key tile jj, half hf, keys of the half
-            struct Cur { int n, jj, hf, valid; };
-            auto cur_keys = [&](const Cur& c) { return min(kSubN, c.valid - c.hf * kSubN); };
-            auto cur_last_half = [&](const Cur& c) { return (c.hf + 1) * kSubN >= c.valid; };
-            auto cur_next = [&](Cur& c) {
-                ++c.n;
-                if (cur_last_half(c)) { ++c.jj; c.hf = 0; c.valid = c.jj < N ? tile_info(c.jj).valid : 0; }
-                else ++c.hf;
-            };
-            auto issue_qk = [&](const Cur& c) {
-                const int i = c.jj % kRingK, t = c.n & 3;
-                if (c.hf == 0) mbar_wait(bar(kBarKFull + i), (c.jj / kRingK) & 1);
-                const int n_cols = (cur_keys(c) + 15) & ~15;  // MMA N (multiple of 16)
-                const uint64_t kd = smem_desc(smem + kOffK + i * kKvTileBytes + (uint32_t)c.hf * (kSubN * 128u), 16, 1024);
-                const uint32_t id_qk = idesc(kTileM, (uint32_t)n_cols, 0);
-                const uint32_t sd = tmem + kTmemS + t * kSubN;
-                tc_fence_after();
-#pragma unroll
-                for (int kk = 0; kk < kD / 16; ++kk) {
-                    const uint64_t off = (uint64_t)(((kk >> 2) * (kQTileBytes / 2) + (kk & 3) * 32) >> 4);
-                    umma_ss(sd, qd + off, kd + off, id_qk, kk > 0);
-                }
-                tc_commit(bar(kBarSFull + t));
-                if (cur_last_half(c)) release(bar(kBarKEmpty + i));  // K is free once the tile's last Q.K^T has completed
-                //@T (c.n < 8 ? 16 + 2 * c.n : 63)
-            };
+            // Every key tile of the chunk is whole (128 keys = two sub-units) except the request's last prefix tile
+            // and its last tree tile.  The issuer loops are the pace-setters of the kernel (one thread, dependent
+            // instructions): no division, no per-tile decode, and the waits of a tile are probed together so that
+            // their latencies (~100-200 clk each even when the phase is long complete) overlap.
+            const int jr0 = wk.np - 1 - wk.j_begin, jr1 = wk.np + wk.nt - 1 - wk.j_begin;
+            const int v0 = wk.L - (wk.np - 1) * kTileN, v1 = wk.T - (wk.nt - 1) * kTileN;
+            auto valid_of = [&](int jj) { return jj == jr0 ? v0 : (jj == jr1 ? v1 : kTileN); };
             if (warp == 18) {
                 // Q.K^T stream: sub-unit n goes out as soon as its S buffer has been read (sub-unit n-4) and its K
                 // tile has landed
                 mbar_wait(bar(kBarQFull), 0);  // (also with N = 0: the CTA must not leave with the load in flight)
-                Cur qc{0, 0, 0, N > 0 ? tile_info(0).valid : 0};
-                while (qc.jj < N) {
-                    if (qc.n >= kTeams) mbar_wait(bar(kBarSFree + (qc.n & 3)), ((qc.n >> 2) & 1) ^ 1);
-                    issue_qk(qc);
-                    cur_next(qc);
+                auto issue_half = [&](uint32_t t, uint32_t ki, uint32_t hf, int keys) {
+                    const int n_cols = (keys + 15) & ~15;  // MMA N (multiple of 16)
+                    const uint64_t kd = smem_desc(smem + kOffK + ki * kKvTileBytes + hf * (kSubN * 128u), 16, 1024);
+                    const uint32_t id_qk = idesc(kTileM, (uint32_t)n_cols, 0);
+                    const uint32_t sd = tmem + kTmemS + t * kSubN;
+                    tc_fence_after();
+#pragma unroll
+                    for (int kk = 0; kk < kD / 16; ++kk) {
+                        const uint64_t off = (uint64_t)(((kk >> 2) * (kQTileBytes / 2) + (kk & 3) * 32) >> 4);
+                        umma_ss(sd, qd + off, kd + off, id_qk, kk > 0);
+                    }
+                    tc_commit(bar(kBarSFull + t));
+                };
+                uint32_t n = 0, ki = 0, kph = 0;
+                for (int jj = 0; jj < N; ++jj) {
+                    const int valid = valid_of(jj);
+                    const bool two = valid > kSubN;
+                    const uint32_t t0 = n & 3, t1 = (n + 1) & 3;
+                    // (a probe that is not needed asks the Q barrier for its long-complete phase 0)
+                    const bool need0 = n >= kTeams, need1 = two && n + 1 >= kTeams;
+                    uint32_t ok_k, ok_0, ok_1;
+                    mbar_probe3(bar(kBarKFull + ki), kph, need0 ? bar(kBarSFree + t0) : bar(kBarQFull),
+                                need0 ? (((n >> 2) & 1) ^ 1) : 0u, need1 ? bar(kBarSFree + t1) : bar(kBarQFull),
+                                need1 ? ((((n + 1) >> 2) & 1) ^ 1) : 0u, ok_k, ok_0, ok_1);
+                    if (!ok_0) mbar_wait(bar(kBarSFree + t0), ((n >> 2) & 1) ^ 1);
+                    if (!ok_k) mbar_wait(bar(kBarKFull + ki), kph);
+                    issue_half(t0, ki, 0, min(valid, kSubN));
+                    if (two) {
+                        if (!ok_1) mbar_wait(bar(kBarSFree + t1), (((n + 1) >> 2) & 1) ^ 1);
+                        issue_half(t1, ki, 1, valid - kSubN);
+                    }
+                    release(bar(kBarKEmpty + ki));  // K is free once the tile's last Q.K^T has completed
+                    n += two ? 2u : 1u;
+                    if (++ki == (uint32_t)kRingK) { ki = 0; kph ^= 1u; }
                 }
             } else {
                 // P.V stream: sub-unit n goes out as its P arrives; the last commit covers every P.V, and every
                 // Q.K^T has completed before its scores were read
-                Cur pc{0, 0, 0, N > 0 ? tile_info(0).valid : 0};
-                uint32_t n_ragged = 0;
-                while (pc.jj < N) {
-                    const int t = pc.n & 3, par = (pc.n >> 2) & 1;
-                    const int vi = pc.jj % kRingV;
-                    if (pc.hf == 0) {
-                        mbar_wait(bar(kBarVFull + vi), (pc.jj / kRingV) & 1);
-                        if (pc.valid & 15) mbar_wait(bar(kBarVFix + n_ragged++), 0);
-                    }
-                    const int ksteps = ((cur_keys(pc) + 15) & ~15) >> 4;  // K extent of this P.V in 16-key steps
+                auto issue_half = [&](uint32_t n, uint32_t vi, uint32_t hf, int keys) {
+                    const uint32_t t = n & 3;
+                    const int ksteps = ((keys + 15) & ~15) >> 4;  // K extent of this P.V in 16-key steps
                     const uint64_t vd = smem_desc(smem + kOffV + vi * kKvTileBytes, kKvTileBytes / 2, 1024);
                     const uint32_t pd = tmem + kTmemP + t * (kSubN / 2);
-                    mbar_wait(bar(kBarPFull + t), par);
                     tc_fence_after();
 #pragma unroll
                     for (int ks = 0; ks < kSubN / 16; ++ks)
                         if (ks < ksteps)
-                            umma_ts(od, pd + ks * 8, vd + (uint64_t)((pc.hf * (kSubN / 16) + ks) * (2048 >> 4)), kIdescPV, (pc.n > 0) | ks);
-                    tc_commit(bar(kBarPFree + (pc.n & 7)));
-                    if (cur_last_half(pc)) release(bar(kBarVEmpty + vi));  // V is free once the tile's last P.V has completed
-                    //@T (pc.n < 8 ? 17 + 2 * pc.n : 63)
-                    cur_next(pc);
+                            umma_ts(od, pd + ks * 8, vd + (uint64_t)((hf * (kSubN / 16) + ks) * (2048 >> 4)), kIdescPV, (n > 0) | ks);
+                    tc_commit(bar(kBarPFree + (n & 7)));
+                };
+                uint32_t n = 0, vi = 0, vph = 0, n_ragged = 0;
+                for (int jj = 0; jj < N; ++jj) {
+                    const int valid = valid_of(jj);
+                    const bool two = valid > kSubN;
+                    uint32_t ok_v, ok_p, ok_x;
+                    mbar_probe3(bar(kBarVFull + vi), vph, bar(kBarPFull + (n & 3)), (n >> 2) & 1, bar(kBarQFull), 0u, ok_v,
+                                ok_p, ok_x);
+                    if (!ok_v) mbar_wait(bar(kBarVFull + vi), vph);
+                    if (valid & 15) mbar_wait(bar(kBarVFix + n_ragged++), 0);
+                    if (!ok_p) mbar_wait(bar(kBarPFull + (n & 3)), (n >> 2) & 1);
+                    issue_half(n, vi, 0, min(valid, kSubN));
+                    if (two) {
+                        mbar_wait(bar(kBarPFull + ((n + 1) & 3)), ((n + 1) >> 2) & 1);
+                        issue_half(n + 1, vi, 1, valid - kSubN);
+                    }
+                    release(bar(kBarVEmpty + vi));  // V is free once the tile's last P.V has completed
+                    n += two ? 2u : 1u;
+                    if (++vi == (uint32_t)kRingV) { vi = 0; vph ^= 1u; }
                 }
                 tc_commit(bar(kBarAllDone));
             }
@@ -565,15 +584,26 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
         const uint32_t sbuf = tmem + kTmemS + t * kSubN + lane_addr;
         const uint32_t pbuf = tmem + kTmemP + t * (kSubN / 2) + lane_addr;
         const int tp = (t + kTeams - 1) & 3;  // the team that owns sub-unit n-1
-        int n = 0, n_sub = 0;                 // n: running sub-unit index; n_sub: total, known after the walk
-        for (int jj = 0; jj < N; ++jj) {
-            const TileInfo ti = tile_info(jj);
-            const int halves = (ti.valid + kSubN - 1) / kSubN;
-            for (int hf = 0; hf < halves; ++hf, ++n) {
-                if ((n & 3) != t) continue;
+        // The sub-unit sequence without a per-tile walk: every key tile of the chunk is whole (two sub-units) except
+        // the request's last prefix tile (chunk-local index jr0, v0 keys) and its last tree tile (jr1, v1 keys; the
+        // last tile of the chunk if it is there at all); a ragged tile of <= 64 keys is a single sub-unit.
+        const int jr0 = wk.np - 1 - wk.j_begin, jr1 = wk.np + wk.nt - 1 - wk.j_begin;
+        const int v0 = wk.L - (wk.np - 1) * kTileN, v1 = wk.T - (wk.nt - 1) * kTileN;
+        const bool in0 = jr0 >= 0 && jr0 < N, in1 = jr1 >= 0 && jr1 < N && jr1 != jr0;
+        const int skip0 = in0 && v0 <= kSubN ? 2 * jr0 : 0x3fffffff;  // sub-units past this index sit one half-tile later
+        const int n_sub = 2 * N - (in0 && v0 <= kSubN ? 1 : 0) - (in1 && v1 <= kSubN ? 1 : 0);
+        const int j_tree = wk.np - wk.j_begin;  // chunk-local index of the first tree tile
+        {
+            for (int n = t; n < n_sub; n += kTeams) {
+                const int n2 = n + (n > skip0 ? 1 : 0);
+                const int jj = n2 >> 1, hf = n2 & 1;
+                struct { int valid; bool tree; int tt; } ti;
+                ti.valid = jj == jr0 ? v0 : (jj == jr1 ? v1 : kTileN);
+                ti.tree = jj >= j_tree;
+                ti.tt = jj - j_tree;
                 const int par = (n >> 2) & 1;
                 const int keys = min(kSubN, ti.valid - hf * kSubN);
-                const bool last = jj == N - 1 && hf == halves - 1;
+                const bool last = n == n_sub - 1;
                 mbar_wait(bar(kBarSFull + t), par);
                 //@T (n < 12 ? 32 + (n >> 2) * 5 : 63)
                 if (!warp_active) {  // a warp without rows only keeps the barrier phases in step
@@ -622,7 +652,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
                 // m_ref(n) to the next team
                 float m_prev = -INFINITY;
                 if (n > 0) {
-                    mbar_wait(bar(kBarRef + 4 * tp + w), ((n - 1) >> 2) & 1);
+                    mbar_wait_warp(lane, bar(kBarRef + 4 * tp + w), ((n - 1) >> 2) & 1);
                     m_prev = xm[tp * kTileM + rl];
                 }
                 const bool need = n > 0 && mx > m_prev + thr;
@@ -632,7 +662,6 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
                     __syncwarp();
                     if (lane == 0) mbar_arrive(bar(kBarRef + 4 * t + w));
                 }
-                //@T (n < 12 ? 34 + (n >> 2) * 5 : 63)
                 if (m_new != m_mine) {  // this thread's own row sum follows the reference
                     l_mine *= m_mine == -INFINITY ? 0.f : ex2((m_mine - m_new) * c2);
                     m_mine = m_new;
@@ -644,7 +673,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
                     // next one cannot be: P.V completions are spread over eight barriers (sub-unit n -> barrier n & 7,
                     // a phase every eight sub-units).  For barrier (n-1) & 7: this thread's own P guard at sub-unit n-4
                     // has seen P.V of n-8 complete, hence n-9 (the P.V stream is in order); P.V of n+7 needs P_n.
-                    mbar_wait(bar(kBarPFree + ((n - 1) & 7)), ((n - 1) >> 3) & 1);
+                    mbar_wait_warp(lane, bar(kBarPFree + ((n - 1) & 7)), ((n - 1) >> 3) & 1);
                     tc_fence_after();
                     const float alpha = need ? (m_prev == -INFINITY ? 0.f : ex2((m_prev - m_new) * c2)) : 1.f;
 #pragma unroll 1
@@ -665,7 +694,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
                 }
                 // the P buffer is free once P.V of sub-unit n-4 has completed (this team sees barriers t and t+4 in
                 // alternation, each phase after phase)
-                if (n >= kTeams) mbar_wait(bar(kBarPFree + ((n - 4) & 7)), ((n - 4) >> 3) & 1);
+                if (n >= kTeams) mbar_wait_warp(lane, bar(kBarPFree + ((n - 4) & 7)), ((n - 4) >> 3) & 1);
                 // a row with every key so far masked has m_ref = -inf: exp2(-inf - 0) = 0, not NaN
                 const float ms = m_new == -INFINITY ? 0.f : m_new * c2;
                 float sum0 = 0.f, sum1 = 0.f;
@@ -695,17 +724,15 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(bar(kBarPFull + t));
-                //@T (n < 12 ? 36 + (n >> 2) * 5 : 63)
             }
         }
-        n_sub = n;
         // ---- epilogue: the four teams' row sums meet at the final reference; the normalised state leaves the
         // CTA straight from registers through a per-warp transpose in shared memory (the rings are free):
         // thread (team t, w, lane) holds columns 32t..32t+31 of row w*32+lane, the warp writes them as whole
         // 32-byte sectors.  A group with a single chunk writes its rows to `out` directly: no exchange. ----
         const int t_last = (n_sub - 1) & 3;
         if (warp_active && n_sub > 0 && t_last == t) xm[t * kTileM + rl] = m_mine;  // owner of the last sub-unit
-        mbar_wait(bar(kBarAllDone), 0);  // every MMA done: O is final, the rings are free
+        mbar_wait_warp(lane, bar(kBarAllDone), 0);  // every MMA done: O is final, the rings are free
         if (pair) asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");  // (see the control warps)
         //@T 56
         named_bar_sync(9, 512);

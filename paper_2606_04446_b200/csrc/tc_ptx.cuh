@@ -38,12 +38,32 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
         : "memory");
     return ok != 0;
 }
+// Three phase tests issued back to back (their latencies overlap); each result is 1 if that phase has completed.
+__device__ __forceinline__ void mbar_probe3(uint32_t b0, uint32_t p0, uint32_t b1, uint32_t p1, uint32_t b2, uint32_t p2,
+                                            uint32_t& ok0, uint32_t& ok1, uint32_t& ok2) {
+    asm volatile(
+        "{\n\t.reg .pred q0, q1, q2;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 q0, [%3], %4;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 q1, [%5], %6;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 q2, [%7], %8;\n\t"
+        "selp.u32 %0, 1, 0, q0;\n\tselp.u32 %1, 1, 0, q1;\n\tselp.u32 %2, 1, 0, q2;\n\t}"
+        : "=r"(ok0), "=r"(ok1), "=r"(ok2)
+        : "r"(b0), "r"(p0), "r"(b1), "r"(p1), "r"(b2), "r"(p2)
+        : "memory");
+}
 // Bounded wait: a protocol bug traps (reported as a launch failure) instead of hanging the GPU.
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     uint32_t spins = 0;
     while (!mbar_try_wait(bar, parity)) {
         if (++spins > (1u << 26)) __trap();
     }
+}
+// The same wait for a whole (converged) warp: one lane polls, the warp meets at a __syncwarp (which also orders the
+// other lanes behind what the poll observed).  32 lanes polling the same barrier are 32 operations in the SM's barrier
+// unit; with 16 such warps spinning, every other barrier operation of the CTA queued ~250 clk behind them.
+__device__ __forceinline__ void mbar_wait_warp(int lane, uint32_t bar, uint32_t parity) {
+    if (lane == 0) mbar_wait(bar, parity);
+    __syncwarp();
 }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
@@ -147,6 +167,16 @@ constexpr uint32_t kIdescPV = idesc(kTileM, kD, 1);
         "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]),   \
         "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])                    \
         : "memory")
+#define D2SD_TMEM_LD16(taddr, r)                                                                            \
+    asm volatile(                                                                                           \
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];" \
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),     \
+          "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]) \
+        : "r"(taddr))
+#define D2SD_TMEM_ST8(taddr, r)                                                                             \
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"r"(taddr),      \
+                 "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7])       \
+                 : "memory")
 // Scheduling fence for 32 registers: the values are "rewritten" here, \
         so everything computed from them
 // stays behind the preceding asm volatile statements (the compiler would otherwise hoist all 128
