@@ -160,6 +160,7 @@ __device__ __forceinline__ void merge_rows(const AttnPlan& pl, const AttnArgs& a
     const int nc = wk.n_chunks;  // <= 64 states
     const size_t grp0 = (size_t)wk.group * pl.grp_rows;
     const int nrows = r1 - r0;  // <= 128
+    const int g_shift = __ffs(G) - 1;  // G divides 128 (attn_stream_supported): a power of two
     constexpr int kSB = 8;      // states per batch
     for (int idx = warp * 32 + lane; idx < nrows * 16; idx += 512) {
         const int r = r0 + (idx >> 4), cg = idx & 15;
@@ -188,8 +189,8 @@ __device__ __forceinline__ void merge_rows(const AttnPlan& pl, const AttnArgs& a
             const float l = lp[(size_t)i * kTileM];
             ws += l == -INFINITY ? 0.f : __expf(l - m);
         }
-        const float inv = ws > 0.f ? 1.f / ws : 0.f;  // no key at all (L = 0, prefix-only mode): O = 0, LSE = -inf
-        const float lse = ws > 0.f ? m + logf(ws) : -INFINITY;
+        const float inv = ws > 0.f ? __fdividef(1.f, ws) : 0.f;  // no key at all (L = 0, prefix-only mode): O = 0, LSE = -inf
+        const float lse = ws > 0.f ? m + __logf(ws) : -INFINITY;  // (1 <= ws <= 64: lg2.approx is accurate to ~1e-7 here)
         float acc[8];
 #pragma unroll
         for (int c = 0; c < 8; ++c) acc[c] = 0.f;
@@ -212,8 +213,8 @@ __device__ __forceinline__ void merge_rows(const AttnPlan& pl, const AttnArgs& a
             acc[4] += w1 * bf_lo(x.z); acc[5] += w1 * bf_hi(x.z);
             acc[6] += w1 * bf_lo(x.w); acc[7] += w1 * bf_hi(x.w);
         }
-        const int ra = wk.row_base + r, t = ra / G;  // query row of the tile -> out / lse row [b][t][h]
-        const size_t orow = ((size_t)wk.b * pl.T_cap + t) * pl.Hq + wk.g * G + (ra - t * G);
+        const int ra = wk.row_base + r, t = ra >> g_shift;  // query row of the tile -> out / lse row [b][t][h]
+        const size_t orow = ((size_t)wk.b * pl.T_cap + t) * pl.Hq + wk.g * G + (ra - (t << g_shift));
         if (dbg_rows) {  // fp32 state for tests
             float* d0 = dbg_rows + orow * (kD + 1) + cg * 8;
 #pragma unroll
@@ -295,17 +296,15 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
     // work decode (the peer has long arrived by then)
     if (pair) asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
     pdl_launch_dependents();  // the next kernel may begin its own prologue as SMs free up
-    pdl_wait();  // everything before this kernel in the stream is complete and visible
-    //@T 2
 
-    // ---- this CTA's work ----
+    // ---- this CTA's work: the part that needs no global memory ----
     Work wk;
+    int n_static;
+    bool pad = false;
     {
-        const int G = pl.G;
         wk.g = blockIdx.y;
         wk.b = blockIdx.z;
-        int x = blockIdx.x, n_static;
-        bool pad = false;
+        int x = blockIdx.x;
         if (pair) {
             const int p = x / (2 * pl.chunks_a), r = x - p * 2 * pl.chunks_a;
             wk.chunk = r >> 1; wk.rank = r & 1; wk.tile = 2 * p + wk.rank; n_static = pl.chunks_a;
@@ -314,21 +313,50 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
             wk.chunk = x; wk.rank = x & 1; wk.tile = pl.n_mt - 1; n_static = pl.chunks_b;
             pad = x >= pl.chunks_b;  // the odd tile's chunk count rounded up to whole clusters
         }
-        wk.T = a.tree_len[wk.b];
-        wk.L = a.ctx_len[wk.b];
-        const int rows_valid = wk.T * G;
         wk.row_base = wk.tile * kTileM;
-        wk.rows = pad ? 0 : max(0, min(kTileM, rows_valid - wk.row_base));
-        // a pair shares its key tiles when both M tiles hold rows (a short tree leaves the odd tile empty)
-        wk.share = pair && rows_valid > (wk.tile | 1) * kTileM;
         wk.group = (wk.b * pl.Hkv + wk.g) * pl.n_mt + wk.tile;
-        wk.np = (mode & 1) ? (wk.L + kTileN - 1) / kTileN : 0;
-        wk.nt = (mode & 2) ? (wk.T + kTileN - 1) / kTileN : 0;
+    }
+    // the chunk's key tiles from the request's lengths
+    auto cut = [&](int T, int L) {
+        wk.T = T;
+        wk.L = L;
+        wk.np = (mode & 1) ? (L + kTileN - 1) / kTileN : 0;
+        wk.nt = (mode & 2) ? (T + kTileN - 1) / kTileN : 0;
         const int nk = wk.np + wk.nt;
         const int tps = max(max(1, pl.tps_min), (nk + n_static - 1) / n_static);
         wk.n_chunks = max(1, (nk + tps - 1) / tps);  // chunk 0 always takes part (nk = 0: state (0, -inf))
         wk.j_begin = wk.chunk * tps;
         wk.n_tiles = max(0, min(nk, wk.j_begin + tps) - wk.j_begin);
+    };
+    // L2 prefetch of the chunk's first ring of K / V tiles, issued BEFORE the grid dependency resolves, from lengths
+    // that may be stale (the preceding kernel may be the one that writes them): a prefetch is a hint, a wrong guess
+    // fetches other lines of the same tensors.  The first tiles' DRAM latency (2.2k-2.9k clk, and the whole
+    // launch asks for its first 9 MB at once) then runs under the dependency wait and the work decode.
+    if (warp == 17 && pl.page_size == 0 && !pad) {
+        int T0, L0, kv0 = 0;
+        asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(T0) : "l"(a.tree_len + wk.b) : "memory");
+        asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(L0) : "l"(a.ctx_len + wk.b) : "memory");
+        if (a.kv_indptr) asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(kv0) : "l"(a.kv_indptr + wk.b) : "memory");
+        if (T0 >= 0 && T0 <= pl.T_cap && L0 >= 0 && L0 <= pl.max_ctx_len) {
+            cut(T0, L0);
+            const int jj = lane >> 1, j = wk.j_begin + jj;
+            const bool v_side = lane & 1;
+            // a sharing pair: rank 0 will load K, rank 1 V (short trees do not share: then both sides are needed
+            // anyway and the other CTA's hint is merely redundant)
+            const bool mine = !pair || wk.rank == (v_side ? 1 : 0);
+            if (lane < 2 * kRingK && jj < wk.n_tiles && j < wk.np && mine)
+                tma_prefetch_4d(v_side ? &tm_v : &tm_k, 0, kv0 + j * kTileN, 0, wk.g);
+        }
+    }
+    pdl_wait();  // everything before this kernel in the stream is complete and visible
+    //@T 2
+    {
+        const int G = pl.G;
+        cut(a.tree_len[wk.b], a.ctx_len[wk.b]);
+        const int rows_valid = wk.T * G;
+        wk.rows = pad ? 0 : max(0, min(kTileM, rows_valid - wk.row_base));
+        // a pair shares its key tiles when both M tiles hold rows (a short tree leaves the odd tile empty)
+        wk.share = pair && rows_valid > (wk.tile | 1) * kTileM;
     }
     // M tiles past the tree's rows, and chunks past the request's key tiles, leave at once:
     // nobody waits for them (n_chunks counts the non-empty chunks only)
@@ -380,7 +408,9 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
             }
             return pg;
         };
-        if (!is_v && lane == 0) {  // Q first: one box = the 128-row query tile of this kv head
+        // Q: one box = the 128-row query tile of this kv head; issued by the V producer (its first tile is needed a
+        // softmax later than the first K tile, and an issue keeps the thread ~400 clk)
+        if (is_v && lane == 0) {
             const int t0 = wk.b * pl.T_cap + wk.row_base / pl.G;
             mbar_expect_tx(bar(kBarQFull), kQTileBytes);
             tma_load_5d(smem + kOffQ, &tm_q, bar(kBarQFull), 0, 0, t0, 0, wk.g, kEvictLast);
@@ -397,7 +427,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
             const bool by_page = paged && !ti.tree;
             const int n_pages = (ti.valid + 15) >> 4;
             if (lane == 0) {
-                mbar_wait(bar(bar_empty + i), round ^ 1u);
+                if (jj >= ring) mbar_wait(bar(bar_empty + i), round ^ 1u);  // (the first fill finds the ring empty)
                 mbar_expect_tx(fb, by_page ? (uint32_t)n_pages * 4096u : kKvTileBytes);
             }
             __syncwarp();
