@@ -72,6 +72,7 @@ constexpr uint32_t kTmemCols = 512;
 constexpr uint32_t kTmemS = 128;   // S_0..S_3 behind O (64 fp32 columns each)
 constexpr uint32_t kTmemP = 384;   // P_0..P_3 (32 columns of bf16 pairs each)
 constexpr float kRescaleThreshold = 8.0f;  // log2 units
+constexpr int kPrefetchTiles = 3;           // key tiles per CTA hinted into L2 in the prologue (measured: 1-3 equal, 4 and 6 slower)
 constexpr uint32_t kRegsControl = 64, kRegsSoftmax = 104;  // setmaxnreg targets: 512 x 104 + 128 x 64 = 60 Ki registers (the launch allocation)
 
 // barrier slots (8 bytes each) at kOffBar
@@ -344,7 +345,7 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
             // a sharing pair: rank 0 will load K, rank 1 V (short trees do not share: then both sides are needed
             // anyway and the other CTA's hint is merely redundant)
             const bool mine = !pair || wk.rank == (v_side ? 1 : 0);
-            if (lane < 2 * kRingK && jj < wk.n_tiles && j < wk.np && mine)
+            if (lane < 2 * kPrefetchTiles && jj < wk.n_tiles && j < wk.np && mine)
                 tma_prefetch_4d(v_side ? &tm_v : &tm_k, 0, kv0 + j * kTileN, 0, wk.g);
         }
     }
