@@ -141,6 +141,17 @@ struct TileInfo {
     int j;          // key tile index within the request (prefix tiles first)
 };
 
+// partial states are read at L2 (written by other SMs; this SM's L1 may hold the previous launch's lines)
+__device__ __forceinline__ float ld_cg_f32(const float* p) {
+    float v;
+    asm volatile("ld.global.cg.f32 %0, [%1];" : "=f"(v) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ uint4 ld_cg_u4(const __nv_bfloat16* p) {
+    uint4 v;
+    asm volatile("ld.global.cg.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
+    return v;
+}
 __device__ __forceinline__ float bf_lo(uint32_t w) { return __uint_as_float(w << 16); }
 __device__ __forceinline__ float bf_hi(uint32_t w) { return __uint_as_float(w & 0xFFFF0000u); }
 
@@ -170,15 +181,15 @@ __device__ __forceinline__ void merge_rows(const AttnPlan& pl, const AttnArgs& a
         float lv[kSB];
         uint4 v[kSB];
 #pragma unroll
-        for (int i = 0; i < kSB; ++i) lv[i] = i < nc ? lp[(size_t)i * kTileM] : -INFINITY;
+        for (int i = 0; i < kSB; ++i) lv[i] = i < nc ? ld_cg_f32(lp + (size_t)i * kTileM) : -INFINITY;
 #pragma unroll
         for (int i = 0; i < kSB; ++i)
-            if (i < nc) v[i] = *reinterpret_cast<const uint4*>(op + (size_t)i * kTileM * kD);
+            if (i < nc) v[i] = ld_cg_u4(op + (size_t)i * kTileM * kD);
         float m = lv[0];
 #pragma unroll
         for (int i = 1; i < kSB; ++i) m = fmaxf(m, lv[i]);
 #pragma unroll 1
-        for (int i = kSB; i < nc; ++i) m = fmaxf(m, lp[(size_t)i * kTileM]);  // more than eight chunks
+        for (int i = kSB; i < nc; ++i) m = fmaxf(m, ld_cg_f32(lp + (size_t)i * kTileM));  // more than eight chunks
         float ws = 0.f, wv[kSB];
 #pragma unroll
         for (int i = 0; i < kSB; ++i) {
@@ -187,7 +198,7 @@ __device__ __forceinline__ void merge_rows(const AttnPlan& pl, const AttnArgs& a
         }
 #pragma unroll 1
         for (int i = kSB; i < nc; ++i) {
-            const float l = lp[(size_t)i * kTileM];
+            const float l = ld_cg_f32(lp + (size_t)i * kTileM);
             ws += l == -INFINITY ? 0.f : __expf(l - m);
         }
         const float inv = ws > 0.f ? __fdividef(1.f, ws) : 0.f;  // no key at all (L = 0, prefix-only mode): O = 0, LSE = -inf
@@ -206,9 +217,9 @@ __device__ __forceinline__ void merge_rows(const AttnPlan& pl, const AttnArgs& a
             }
 #pragma unroll 1
         for (int i = kSB; i < nc; ++i) {
-            const float l = lp[(size_t)i * kTileM];
+            const float l = ld_cg_f32(lp + (size_t)i * kTileM);
             const float w1 = l == -INFINITY ? 0.f : __expf(l - m) * inv;
-            const uint4 x = *reinterpret_cast<const uint4*>(op + (size_t)i * kTileM * kD);
+            const uint4 x = ld_cg_u4(op + (size_t)i * kTileM * kD);
             acc[0] += w1 * bf_lo(x.x); acc[1] += w1 * bf_hi(x.x);
             acc[2] += w1 * bf_lo(x.y); acc[3] += w1 * bf_hi(x.y);
             acc[4] += w1 * bf_lo(x.z); acc[5] += w1 * bf_hi(x.z);
@@ -875,7 +886,9 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
                             }
                         }
                     } while (seen < expected);
-                    __threadfence();  // acquire side: the states are read with ordinary loads behind the barrier below
+                    // acquire side: one acquire load of the counter (lighter than a full fence: nothing of this thread's
+                    // own is outstanding); the states are read at L2 (ld.global.cg) behind the barrier below
+                    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(cnt) : "memory");
                     // this CTA is past the wait: count it out now, the round trip hides behind the merge
                     done_before = atomicAdd(cnt + 1, 1u);
                     xl[0] = __int_as_float(ok);
