@@ -751,20 +751,24 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
         // thread (team t, w, lane) holds columns 32t..32t+31 of row w*32+lane, the warp writes them as whole
         // 32-byte sectors.  A group with a single chunk writes its rows to `out` directly: no exchange. ----
         const int t_last = (n_sub - 1) & 3;
-        if (warp_active && n_sub > 0 && t_last == t) xm[t * kTileM + rl] = m_mine;  // owner of the last sub-unit
         mbar_wait_warp(lane, bar(kBarAllDone), 0);  // every MMA done: O is final, the rings are free
         if (pair) asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");  // (see the control warps)
         //@T 56
+        // every team's (reference, row sum) of the row through the free V ring, one barrier: the final reference
+        // is the one of the last sub-unit's owner, each sum is brought to it
+        float2* xp = reinterpret_cast<float2*>(smem_gen + kOffV);
+        float* xl = reinterpret_cast<float*>(smem_gen + kOffXL);  // (scratch word of the group wait below)
+        xp[t * kTileM + rl] = make_float2(m_mine, l_mine);
         named_bar_sync(9, 512);
-        const float m_fin = n_sub > 0 ? xm[t_last * kTileM + rl] : -INFINITY;
-        if (m_fin != m_mine) l_mine *= m_mine == -INFINITY ? 0.f : ex2((m_mine - m_fin) * c2);
-        named_bar_sync(10, 512);  // everybody has read the final reference: the row sums take its place
-        float* xl = reinterpret_cast<float*>(smem_gen + kOffXL);
-        xl[t * kTileM + rl] = l_mine;
-        named_bar_sync(9, 512);
-        const float l_tot = (xl[rl] + xl[kTileM + rl]) + (xl[2 * kTileM + rl] + xl[3 * kTileM + rl]);
-        const float inv = l_tot > 0.f ? 1.f / l_tot : 0.f;  // l = 0: every key of the chunk masked, or no key at all
-        const float lse_v = l_tot > 0.f ? m_fin * pl.sm_scale + logf(l_tot) : -INFINITY;
+        const float m_fin = n_sub > 0 ? xp[t_last * kTileM + rl].x : -INFINITY;
+        float l_tot = 0.f;
+#pragma unroll
+        for (int tt = 0; tt < kTeams; ++tt) {
+            const float2 ml = xp[tt * kTileM + rl];
+            l_tot += ml.x == -INFINITY ? 0.f : ml.y * (ml.x == m_fin ? 1.f : ex2((ml.x - m_fin) * c2));
+        }
+        const float inv = l_tot > 0.f ? __fdividef(1.f, l_tot) : 0.f;  // l = 0: every key of the chunk masked, or no key at all
+        const float lse_v = l_tot > 0.f ? m_fin * pl.sm_scale + __logf(l_tot) : -INFINITY;
         //@T 57
         const bool direct = wk.n_chunks == 1;
         const bool row_ok = rl < wk.rows;
