@@ -93,9 +93,15 @@ struct TileInfo {
     int j;          // key tile index within the request (prefix tiles first)
 };
 
-__device__ __forceinline__ uint2 ld_cg_u2(const __nv_bfloat16* p) {
-    uint2 v;
-    asm volatile("ld.global.v2.u32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "l"(p));
+// partial states are read at L2 (written by other SMs; this SM's L1 may hold the previous launch's lines)
+__device__ __forceinline__ float ld_cg_f32(const float* p) {
+    float v;
+    asm volatile("ld.global.cg.f32 %0, [%1];" : "=f"(v) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ uint4 ld_cg_u4(const __nv_bfloat16* p) {
+    uint4 v;
+    asm volatile("ld.global.cg.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
     return v;
 }
 __device__ __forceinline__ float bf_lo(uint32_t w) { return __uint_as_float(w << 16); }
@@ -104,102 +110,89 @@ __device__ __forceinline__ float bf_hi(uint32_t w) { return __uint_as_float(w & 
 // -------------------------------------------------------------------------------------------------
 // Cascade merge of one group's rows (log-sum-exp state merge):
 //   LSE = log sum_p e^{LSE_p};  O = sum_p e^{LSE_p - LSE} O_p   over the group's chunk states.
-// CTA `chunk` of the group's n_chunks CTAs takes a contiguous range of the item's rows; a warp takes
-// two rows at a time.  Everything a warp needs for its rows is requested at once -- lane i loads the
-// LSE of state i, every lane loads its 16-byte piece of every state's O row (512 contiguous bytes per
-// warp instruction, up to eight states x two rows in flight) -- so the merge costs one L2 round trip;
-// the weights are reduced with shuffles and never leave the registers.  The partial states were written
-// by other SMs and published with a release; they are read at L2 (ld.global.cg).
+// CTA `chunk` of the group's n_chunks CTAs takes a contiguous range of the item's rows.  One THREAD takes 8
+// columns of one row (16 threads a row, 512 threads = 32 rows a pass): it loads the row's LSE of every state and
+// its 16-byte piece of every state's O row (all requested at once: one L2 round trip), forms the weights itself
+// (no shuffles) and writes 16 bytes of the output.  The decomposition matters more than the traffic: a warp
+// executes a dependent instruction every 5-8 clk, so the merge costs (instructions per thread) x that, and the
+// earlier warp-per-two-rows form (shuffled weights, ~600 instructions per thread) took 4.6k-8.6k clk.
+// The partial states were written by other SMs and published with a release; the loads follow the group wait's
+// acquire fence.
 __device__ __forceinline__ void merge_rows(const AttnPlan& pl, const AttnArgs& a, float* dbg_rows, const Work& wk,
                                            int r0, int r1, int warp, int lane) {
     const int G = pl.G;
     const int nc = wk.n_chunks;  // <= 64 states
     const size_t grp0 = (size_t)wk.group * pl.grp_rows;
-    const int nrows = r1 - r0;  // <= 128
-    constexpr int kRB = 2, kSB = 8;
-    for (int rb = warp * kRB; rb < nrows; rb += 16 * kRB) {
-        // lane i holds LSE of states i and i + 32 for each of the two rows
-        float lv[kRB][2];
+    const int nrows = r1 - r0;  // <= 256
+    const int g_shift = __ffs(G) - 1;  // G divides 128 (attn_duo_supported): a power of two
+    constexpr int kSB = 8;      // states per batch
+    for (int idx = warp * 32 + lane; idx < nrows * 16; idx += 512) {
+        const int r = r0 + (idx >> 4), cg = idx & 15;
+        const float* lp = a.part_lse + grp0 + r;
+        const __nv_bfloat16* op = a.part_o16 + (grp0 + r) * kD + cg * 8;
+        float lv[kSB];
+        uint4 v[kSB];
 #pragma unroll
-        for (int u = 0; u < kRB; ++u)
+        for (int i = 0; i < kSB; ++i) lv[i] = i < nc ? ld_cg_f32(lp + (size_t)i * kItemRows) : -INFINITY;
 #pragma unroll
-            for (int hh = 0; hh < 2; ++hh) {
-                const int i = lane + 32 * hh;
-                lv[u][hh] = (rb + u < nrows && i < nc) ? a.part_lse[grp0 + (size_t)i * kItemRows + r0 + rb + u] : -INFINITY;
+        for (int i = 0; i < kSB; ++i)
+            if (i < nc) v[i] = ld_cg_u4(op + (size_t)i * kItemRows * kD);
+        float m = lv[0];
+#pragma unroll
+        for (int i = 1; i < kSB; ++i) m = fmaxf(m, lv[i]);
+#pragma unroll 1
+        for (int i = kSB; i < nc; ++i) m = fmaxf(m, ld_cg_f32(lp + (size_t)i * kItemRows));  // more than eight chunks
+        float ws = 0.f, wv[kSB];
+#pragma unroll
+        for (int i = 0; i < kSB; ++i) {
+            wv[i] = lv[i] == -INFINITY ? 0.f : __expf(lv[i] - m);
+            ws += wv[i];
+        }
+#pragma unroll 1
+        for (int i = kSB; i < nc; ++i) {
+            const float l = ld_cg_f32(lp + (size_t)i * kItemRows);
+            ws += l == -INFINITY ? 0.f : __expf(l - m);
+        }
+        const float inv = ws > 0.f ? __fdividef(1.f, ws) : 0.f;  // no key at all (L = 0, prefix-only mode): O = 0, LSE = -inf
+        const float lse = ws > 0.f ? m + __logf(ws) : -INFINITY;  // (1 <= ws <= 64: lg2.approx is accurate to ~1e-7 here)
+        float acc[8];
+#pragma unroll
+        for (int c = 0; c < 8; ++c) acc[c] = 0.f;
+#pragma unroll
+        for (int i = 0; i < kSB; ++i)
+            if (i < nc) {  // states without any key hold zeros (their CTA wrote them)
+                const float w1 = wv[i] * inv;
+                acc[0] += w1 * bf_lo(v[i].x); acc[1] += w1 * bf_hi(v[i].x);
+                acc[2] += w1 * bf_lo(v[i].y); acc[3] += w1 * bf_hi(v[i].y);
+                acc[4] += w1 * bf_lo(v[i].z); acc[5] += w1 * bf_hi(v[i].z);
+                acc[6] += w1 * bf_lo(v[i].w); acc[7] += w1 * bf_hi(v[i].w);
             }
-        uint2 v[kRB][kSB];
-#pragma unroll
-        for (int u = 0; u < kRB; ++u)
-#pragma unroll
-            for (int i = 0; i < kSB; ++i)
-                if (rb + u < nrows && i < nc)
-                    v[u][i] = ld_cg_u2(a.part_o16 + (grp0 + (size_t)i * kItemRows + r0 + rb + u) * kD + lane * 4);
-                float wv[kRB][2], lse[kRB];
-#pragma unroll
-        for (int u = 0; u < kRB; ++u) {
-            float m = fmaxf(lv[u][0], lv[u][1]);
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
-            wv[u][0] = lv[u][0] == -INFINITY ? 0.f : __expf(lv[u][0] - m);
-            wv[u][1] = lv[u][1] == -INFINITY ? 0.f : __expf(lv[u][1] - m);
-            float ws = wv[u][0] + wv[u][1];
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) ws += __shfl_xor_sync(0xffffffffu, ws, o);
-            const float inv = ws > 0.f ? 1.f / ws : 0.f;  // no key at all (L = 0, prefix-only mode): O = 0, LSE = -inf
-            wv[u][0] *= inv;
-            wv[u][1] *= inv;
-            lse[u] = ws > 0.f ? m + logf(ws) : -INFINITY;
+#pragma unroll 1
+        for (int i = kSB; i < nc; ++i) {
+            const float l = ld_cg_f32(lp + (size_t)i * kItemRows);
+            const float w1 = l == -INFINITY ? 0.f : __expf(l - m) * inv;
+            const uint4 x = ld_cg_u4(op + (size_t)i * kItemRows * kD);
+            acc[0] += w1 * bf_lo(x.x); acc[1] += w1 * bf_hi(x.x);
+            acc[2] += w1 * bf_lo(x.y); acc[3] += w1 * bf_hi(x.y);
+            acc[4] += w1 * bf_lo(x.z); acc[5] += w1 * bf_hi(x.z);
+            acc[6] += w1 * bf_lo(x.w); acc[7] += w1 * bf_hi(x.w);
         }
-        float4 acc[kRB];
+        const int ra = wk.row_base + r, t = ra >> g_shift;  // query row of the tile -> out / lse row [b][t][h]
+        const size_t orow = ((size_t)wk.b * pl.T_cap + t) * pl.Hq + wk.g * G + (ra - (t << g_shift));
+        if (dbg_rows) {  // fp32 state for tests
+            float* d0 = dbg_rows + orow * (kD + 1) + cg * 8;
 #pragma unroll
-        for (int u = 0; u < kRB; ++u) {
-            acc[u] = make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll
-            for (int i = 0; i < kSB; ++i) {
-                const float w1 = __shfl_sync(0xffffffffu, wv[u][0], i);
-                if (rb + u < nrows && i < nc) {  // states without any key hold zeros (their CTA wrote them)
-                    acc[u].x += w1 * bf_lo(v[u][i].x); acc[u].y += w1 * bf_hi(v[u][i].x);
-                    acc[u].z += w1 * bf_lo(v[u][i].y); acc[u].w += w1 * bf_hi(v[u][i].y);
-                }
-            }
+            for (int c = 0; c < 8; ++c) d0[c] = acc[c];
+            if (cg == 0) dbg_rows[orow * (kD + 1) + kD] = lse;
+            continue;
         }
-        for (int s0 = kSB; s0 < nc; s0 += kSB) {  // more than eight chunks: further batches of states
-#pragma unroll
-            for (int u = 0; u < kRB; ++u)
-#pragma unroll
-                for (int i = 0; i < kSB; ++i)
-                    if (rb + u < nrows && s0 + i < nc)
-                        v[u][i] = ld_cg_u2(a.part_o16 + (grp0 + (size_t)(s0 + i) * kItemRows + r0 + rb + u) * kD + lane * 4);
-#pragma unroll
-            for (int u = 0; u < kRB; ++u)
-#pragma unroll
-                for (int i = 0; i < kSB; ++i) {
-                    const int st = s0 + i;
-                    const float wa = __shfl_sync(0xffffffffu, wv[u][0], st & 31), wb = __shfl_sync(0xffffffffu, wv[u][1], st & 31);
-                    const float w1 = st < 32 ? wa : wb;
-                    if (rb + u < nrows && st < nc) {
-                        acc[u].x += w1 * bf_lo(v[u][i].x); acc[u].y += w1 * bf_hi(v[u][i].x);
-                        acc[u].z += w1 * bf_lo(v[u][i].y); acc[u].w += w1 * bf_hi(v[u][i].y);
-                    }
-                }
-        }
-#pragma unroll
-        for (int u = 0; u < kRB; ++u) {
-            if (rb + u >= nrows) continue;
-            const int ra = wk.row_base + r0 + rb + u, t = ra / G;  // query row of the tile -> out / lse row [b][t][h]
-            const size_t orow = ((size_t)wk.b * pl.T_cap + t) * pl.Hq + wk.g * G + (ra - t * G);
-            if (dbg_rows) {  // fp32 state for tests
-                float* d0 = dbg_rows + orow * (kD + 1) + lane * 4;
-                d0[0] = acc[u].x; d0[1] = acc[u].y; d0[2] = acc[u].z; d0[3] = acc[u].w;
-                if (lane == 0) dbg_rows[orow * (kD + 1) + kD] = lse[u];
-                continue;
-            }
-            uint2 pk;
-            pk.x = pack2_bf16(acc[u].x, acc[u].y);
-            pk.y = pack2_bf16(acc[u].z, acc[u].w);
-            *reinterpret_cast<uint2*>(a.out + orow * kD + lane * 4) = pk;
-            if (lane == 0 && a.lse) a.lse[orow] = lse[u];
-        }
+        uint4 pk;
+        pk.x = pack2_bf16(acc[0], acc[1]);
+        pk.y = pack2_bf16(acc[2], acc[3]);
+        pk.z = pack2_bf16(acc[4], acc[5]);
+        pk.w = pack2_bf16(acc[6], acc[7]);
+        *reinterpret_cast<uint4*>(a.out + orow * kD + cg * 8) = pk;
+        if (cg == 0 && a.lse) a.lse[orow] = lse;
     }
 }
 
@@ -388,11 +381,16 @@ attn_duo_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
         // released by the commit behind its last reader. =====
         if (elect_one()) {
             const int per = 2 * n_m;  // sub-units per key tile: n -> (key tile n / per, half (n % per) / n_m, M tile n % n_m)
-            auto keys_of = [&](int jj, int hf) { return max(0, min(kSubN, tile_info(jj).valid - hf * kSubN)); };
+            // (per is 2 or 4: shifts; every key tile is whole except the request's last prefix and last tree tile:
+            // the issuer threads pace the kernel, see attn_stream_sm100.cu)
+            const int jr0 = wk.np - 1 - wk.j_begin, jr1 = wk.np + wk.nt - 1 - wk.j_begin;
+            const int v0 = wk.L - (wk.np - 1) * kTileN, v1 = wk.T - (wk.nt - 1) * kTileN;
+            auto valid_of = [&](int jj) { return jj == jr0 ? v0 : (jj == jr1 ? v1 : kTileN); };
+            auto keys_of = [&](int jj, int hf) { return max(0, min(kSubN, valid_of(jj) - hf * kSubN)); };
             if (warp == 18) {
                 for (int m = 0; m < n_m; ++m) mbar_wait(bar(kBarQFull + m), 0);  // (also with N = 0: no load left in flight)
                 for (int n = 0; n < n_sub; ++n) {
-                    const int jj = n / per, r = n - jj * per, hf = r / n_m, m = r - hf * n_m, t = n & 3;
+                    const int jj = n >> n_m, r = n & (per - 1), hf = r >> (n_m - 1), m = r & (n_m - 1), t = n & 3;
                     const int i = jj % kRingK;
                     if (r == 0) mbar_wait(bar(kBarKFull + i), (jj / kRingK) & 1);
                     if (n >= kTeams) mbar_wait(bar(kBarPFree + t), ((n >> 2) & 1) ^ 1);  // P.V of n-4 has consumed the buffer
@@ -415,12 +413,12 @@ attn_duo_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
             } else {
                 uint32_t n_ragged = 0, started = 0;  // started: bit m set once O_m holds a product
                 for (int n = 0; n < n_sub; ++n) {
-                    const int jj = n / per, r = n - jj * per, hf = r / n_m, m = r - hf * n_m, t = n & 3;
+                    const int jj = n >> n_m, r = n & (per - 1), hf = r >> (n_m - 1), m = r & (n_m - 1), t = n & 3;
                     const int vi = jj % kRingV;
                     const int keys = keys_of(jj, hf);
                     if (r == 0) {
                         mbar_wait(bar(kBarVFull + vi), (jj / kRingV) & 1);
-                        if (tile_info(jj).valid & 15) mbar_wait(bar(kBarVFix + n_ragged++), 0);
+                        if (valid_of(jj) & 15) mbar_wait(bar(kBarVFix + n_ragged++), 0);
                     }
                     const int ksteps = ((keys + 15) & ~15) >> 4;  // K extent of this P.V in 16-key steps
                     const uint64_t vd = smem_desc(smem + kOffV + vi * kKvTileBytes, kKvTileBytes / 2, 1024);
@@ -465,10 +463,15 @@ attn_duo_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
         const uint32_t* mrow = a.mask + ((size_t)wk.b * pl.T_cap + t_node) * pl.W;
         const uint32_t sbuf = tmem + kTmemBuf + t * kSubN + lane_addr;
         const uint32_t o_addr = tmem + m * kD + lane_addr;
+        const int s_jr0 = wk.np - 1 - wk.j_begin, s_jr1 = wk.np + wk.nt - 1 - wk.j_begin, s_jtree = wk.np - wk.j_begin;
+        const int s_v0 = wk.L - (wk.np - 1) * kTileN, s_v1 = wk.T - (wk.nt - 1) * kTileN;
         for (int n = t; n < n_sub; n += kTeams) {
-            const int jj = n / per, r = n - jj * per, hf = r / n_m;
+            const int jj = n >> n_m, r = n & (per - 1), hf = r >> (n_m - 1);
             const int par = (n >> 2) & 1;
-            const TileInfo ti = tile_info(jj);
+            struct { int valid; bool tree; int tt; } ti;  // (no per-tile decode: see the issuers)
+            ti.valid = jj == s_jr0 ? s_v0 : (jj == s_jr1 ? s_v1 : kTileN);
+            ti.tree = jj >= s_jtree;
+            ti.tt = jj - s_jtree;
             const int keys = max(0, min(kSubN, ti.valid - hf * kSubN));
             // the M tile's previous sub-unit is n - n_m (the sequence is (h0: m0 [m1]) (h1: m0 [m1]) per key tile)
             const int n_prev = n - n_m;
@@ -724,7 +727,9 @@ attn_duo_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
                             }
                         }
                     } while (seen < expected);
-                    __threadfence();  // acquire side: the states are read with ordinary loads behind the barrier below
+                    // acquire side: one acquire load of the counter; the states are read at L2 (ld.global.cg) behind
+                    // the barrier below
+                    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(cnt) : "memory");
                     done_before = atomicAdd(cnt + 1, 1u);
                     xl[0] = __int_as_float(ok);
                 }
