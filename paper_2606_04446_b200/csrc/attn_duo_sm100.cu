@@ -389,52 +389,72 @@ attn_duo_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
             auto keys_of = [&](int jj, int hf) { return max(0, min(kSubN, valid_of(jj) - hf * kSubN)); };
             if (warp == 18) {
                 for (int m = 0; m < n_m; ++m) mbar_wait(bar(kBarQFull + m), 0);  // (also with N = 0: no load left in flight)
-                for (int n = 0; n < n_sub; ++n) {
-                    const int jj = n >> n_m, r = n & (per - 1), hf = r >> (n_m - 1), m = r & (n_m - 1), t = n & 3;
-                    const int i = jj % kRingK;
-                    if (r == 0) mbar_wait(bar(kBarKFull + i), (jj / kRingK) & 1);
-                    if (n >= kTeams) mbar_wait(bar(kBarPFree + t), ((n >> 2) & 1) ^ 1);  // P.V of n-4 has consumed the buffer
-                    int n_cols = (keys_of(jj, hf) + 15) & ~15;  // MMA N (multiple of 16); an empty half still produces
-                    if (n_cols == 0) n_cols = 16;               // 16 columns that are all masked
-                    const uint64_t qd = smem_desc(smem + kOffQ + m * kQTileBytes, 16, 1024);
-                    const uint64_t kd = smem_desc(smem + kOffK + i * kKvTileBytes + (uint32_t)hf * (kSubN * 128u), 16, 1024);
-                    const uint32_t id_qk = idesc(kTileM, (uint32_t)n_cols, 0);
-                    const uint32_t sd = tmem + kTmemBuf + t * kSubN;
-                    tc_fence_after();
+                uint32_t n = 0, ki = 0, kph = 0;
+                for (int jj = 0; jj < N; ++jj) {
+                    const int valid = valid_of(jj);
+                    // the tile's K barrier and the buffers of its first two sub-units, probed together
+                    uint32_t ok_k, ok_0, ok_1;
+                    mbar_probe3(bar(kBarKFull + ki), kph, n >= kTeams ? bar(kBarPFree + (n & 3)) : bar(kBarQFull),
+                                n >= kTeams ? (((n >> 2) & 1) ^ 1) : 0u,
+                                n + 1 >= kTeams ? bar(kBarPFree + ((n + 1) & 3)) : bar(kBarQFull),
+                                n + 1 >= kTeams ? ((((n + 1) >> 2) & 1) ^ 1) : 0u, ok_k, ok_0, ok_1);
+                    if (!ok_k) mbar_wait(bar(kBarKFull + ki), kph);
+                    const uint64_t kd0 = smem_desc(smem + kOffK + ki * kKvTileBytes, 16, 1024);
+#pragma unroll 1
+                    for (int r = 0; r < per; ++r, ++n) {
+                        const int hf = r >> (n_m - 1), m = r & (n_m - 1);
+                        const uint32_t t = n & 3;
+                        // P.V of n-4 has consumed the buffer
+                        if (n >= kTeams && !(r == 0 ? ok_0 : (r == 1 ? ok_1 : 0u)))
+                            mbar_wait(bar(kBarPFree + t), ((n >> 2) & 1) ^ 1);
+                        int n_cols = (max(0, min(kSubN, valid - hf * kSubN)) + 15) & ~15;  // MMA N (multiple of 16); an empty
+                        if (n_cols == 0) n_cols = 16;  // half still produces 16 columns that are all masked
+                        const uint64_t qd = smem_desc(smem + kOffQ + m * kQTileBytes, 16, 1024);
+                        const uint64_t kd = kd0 + (uint64_t)((hf * (kSubN * 128u)) >> 4);
+                        const uint32_t id_qk = idesc(kTileM, (uint32_t)n_cols, 0);
+                        const uint32_t sd = tmem + kTmemBuf + t * kSubN;
+                        tc_fence_after();
 #pragma unroll
-                    for (int kk = 0; kk < kD / 16; ++kk) {
-                        const uint64_t off = (uint64_t)(((kk >> 2) * (kQTileBytes / 2) + (kk & 3) * 32) >> 4);
-                        umma_ss(sd, qd + off, kd + off, id_qk, kk > 0);
+                        for (int kk = 0; kk < kD / 16; ++kk) {
+                            const uint64_t off = (uint64_t)(((kk >> 2) * (kQTileBytes / 2) + (kk & 3) * 32) >> 4);
+                            umma_ss(sd, qd + off, kd + off, id_qk, kk > 0);
+                        }
+                        tc_commit(bar(kBarSFull + t));
                     }
-                    tc_commit(bar(kBarSFull + t));
-                    if (r == per - 1) tc_commit(bar(kBarKEmpty + i));  // K is free once the tile's last Q.K^T has completed
-                    //@T ((n - TL_N0) >= 0 && (n - TL_N0) < 8 ? 16 + 2 * (n - TL_N0) : 63)
+                    tc_commit(bar(kBarKEmpty + ki));  // K is free once the tile's last Q.K^T has completed
+                    if (++ki == (uint32_t)kRingK) { ki = 0; kph ^= 1u; }
                 }
             } else {
                 uint32_t n_ragged = 0, started = 0;  // started: bit m set once O_m holds a product
-                for (int n = 0; n < n_sub; ++n) {
-                    const int jj = n >> n_m, r = n & (per - 1), hf = r >> (n_m - 1), m = r & (n_m - 1), t = n & 3;
-                    const int vi = jj % kRingV;
-                    const int keys = keys_of(jj, hf);
-                    if (r == 0) {
-                        mbar_wait(bar(kBarVFull + vi), (jj / kRingV) & 1);
-                        if (valid_of(jj) & 15) mbar_wait(bar(kBarVFix + n_ragged++), 0);
-                    }
-                    const int ksteps = ((keys + 15) & ~15) >> 4;  // K extent of this P.V in 16-key steps
+                uint32_t n = 0, vi = 0, vph = 0;
+                for (int jj = 0; jj < N; ++jj) {
+                    const int valid = valid_of(jj);
+                    uint32_t ok_v, ok_p, ok_x;
+                    mbar_probe3(bar(kBarVFull + vi), vph, bar(kBarPFull + (n & 3)), (n >> 2) & 1, bar(kBarQFull), 0u, ok_v,
+                                ok_p, ok_x);
+                    if (!ok_v) mbar_wait(bar(kBarVFull + vi), vph);
+                    if (valid & 15) mbar_wait(bar(kBarVFix + n_ragged++), 0);
                     const uint64_t vd = smem_desc(smem + kOffV + vi * kKvTileBytes, kKvTileBytes / 2, 1024);
-                    const uint32_t pd = tmem + kTmemBuf + t * kSubN;
-                    const uint32_t od = tmem + m * kD;
-                    mbar_wait(bar(kBarPFull + t), (n >> 2) & 1);
-                    tc_fence_after();
+#pragma unroll 1
+                    for (int r = 0; r < per; ++r, ++n) {
+                        const int hf = r >> (n_m - 1), m = r & (n_m - 1);
+                        const uint32_t t = n & 3;
+                        const int keys = max(0, min(kSubN, valid - hf * kSubN));
+                        const int ksteps = ((keys + 15) & ~15) >> 4;  // K extent of this P.V in 16-key steps
+                        const uint32_t pd = tmem + kTmemBuf + t * kSubN;
+                        const uint32_t od = tmem + m * kD;
+                        if (!(r == 0 && ok_p)) mbar_wait(bar(kBarPFull + t), (n >> 2) & 1);
+                        tc_fence_after();
 #pragma unroll
-                    for (int ks = 0; ks < kSubN / 16; ++ks)
-                        if (ks < ksteps)
-                            umma_ts(od, pd + ks * 8, vd + (uint64_t)((hf * (kSubN / 16) + ks) * (2048 >> 4)), kIdescPV,
-                                    ((started >> m) & 1u) | ks);
-                    if (ksteps > 0) started |= 1u << m;
-                    tc_commit(bar(kBarPFree + t));
-                    if (r == per - 1) tc_commit(bar(kBarVEmpty + vi));  // V is free once the tile's last P.V has completed
-                    //@T ((n - TL_N0) >= 0 && (n - TL_N0) < 8 ? 17 + 2 * (n - TL_N0) : 63)
+                        for (int ks = 0; ks < kSubN / 16; ++ks)
+                            if (ks < ksteps)
+                                umma_ts(od, pd + ks * 8, vd + (uint64_t)((hf * (kSubN / 16) + ks) * (2048 >> 4)), kIdescPV,
+                                        ((started >> m) & 1u) | ks);
+                        if (ksteps > 0) started |= 1u << m;
+                        tc_commit(bar(kBarPFree + t));
+                    }
+                    tc_commit(bar(kBarVEmpty + vi));  // V is free once the tile's last P.V has completed
+                    if (++vi == (uint32_t)kRingV) { vi = 0; vph ^= 1u; }
                 }
                 tc_commit(bar(kBarAllDone));
             }
