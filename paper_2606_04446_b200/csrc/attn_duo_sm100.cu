@@ -211,7 +211,6 @@ attn_duo_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
     auto bar = [&](uint32_t i) { return bar0 + 8u * i; };
     volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(smem_gen + kOffBar + 8u * kTmemSlot);
 
-    //@T 0
     // ---- prologue that touches no global memory (overlaps the preceding kernel's tail under PDL) ----
     if (warp == 16 && lane == 0) {
         mbar_init(bar(kBarQFull + 0), 1);
@@ -498,7 +497,6 @@ attn_duo_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
             const bool has_prev = n_prev >= 0;
             const bool has_next = n + n_m < n_sub;
             mbar_wait(bar(kBarSFull + t), par);
-            //@T ((n - TL_N0) >= 0 && (n - TL_N0) < 12 ? 32 + ((n - TL_N0) >> 2) * 5 : 63)
             if (!warp_active) {  // a warp without rows only keeps the barrier phases in step
                 if (lane == 0) mbar_arrive(bar(kBarPFull + t));
                 __syncwarp();
@@ -533,7 +531,6 @@ attn_duo_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
                 mx3 = fmaxf(mx3, __uint_as_float(sv[c + 3]));
             }
             const float mx = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
-            //@T ((n - TL_N0) >= 0 && (n - TL_N0) < 12 ? 33 + ((n - TL_N0) >> 2) * 5 : 63)
             // reference hand-off along the M tile's sub-unit sequence, lazy raise
             float m_prev = -INFINITY;
             if (has_prev) {
@@ -547,7 +544,6 @@ attn_duo_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
                 __syncwarp();
                 if (lane == 0) mbar_arrive(bar(kBarRef + 4 * t + w));
             }
-            //@T ((n - TL_N0) >= 0 && (n - TL_N0) < 12 ? 34 + ((n - TL_N0) >> 2) * 5 : 63)
             if (m_new != m_mine) {  // this thread's own row sum follows the reference
                 l_mine *= m_mine == -INFINITY ? 0.f : ex2((m_mine - m_new) * c2);
                 m_mine = m_new;
@@ -605,7 +601,6 @@ attn_duo_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(bar(kBarPFull + t));
-            //@T ((n - TL_N0) >= 0 && (n - TL_N0) < 12 ? 36 + ((n - TL_N0) >> 2) * 5 : 63)
         }
         // ---- epilogue: the row sums of the teams that share an M tile meet at the final reference; the normalised
         // state leaves the CTA straight from registers through a per-warp transpose in shared memory (the rings
@@ -770,7 +765,6 @@ attn_duo_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
 
     tc_fence_before();
     __syncthreads();
-    //@T 62
     if (warp == 18) {
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(kTmemCols) : "memory");
     }

@@ -50,7 +50,13 @@
 // linear order.  A wait that does not end sets an error word in the workspace header instead of
 // trapping (d2sd.h).
 // The launch is a programmatic dependent launch: the prologue (barriers, TMEM, tensor-map prefetch)
-// overlaps the tail of the preceding kernel; no global memory is touched before griddepcontrol.wait.
+// overlaps the tail of the preceding kernel.  Before griddepcontrol.wait nothing is read for use and nothing is
+// written: one warp reads the request's lengths as they stand (possibly stale) only to aim an L2 prefetch hint at
+// the chunk's first K / V tiles; every value the kernel computes with is read after the wait.
+// Pace: one-thread roles (the two MMA issuers, the producers) and one-shot code (prologue, epilogue) cost
+// (instructions) x 5-8 clk, and a barrier test keeps a thread 100-250 clk; they, not the softmax warps, set the
+// kernel's pace (profiles/r02_experiments.md, "Per-thread timeline"), so their loops carry their state incrementally
+// (no division, no per-tile decode) and probe the barriers of a tile together.
 #include "tc_ptx.cuh"
 
 namespace d2sd {
@@ -303,7 +309,6 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
-    //@T 1
     // the peer's barriers must be initialised before anything remote reaches them: arrive now, wait after the
     // work decode (the peer has long arrived by then)
     if (pair) asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
@@ -361,7 +366,6 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
         }
     }
     pdl_wait();  // everything before this kernel in the stream is complete and visible
-    //@T 2
     {
         const int G = pl.G;
         cut(a.tree_len[wk.b], a.ctx_len[wk.b]);
@@ -385,7 +389,6 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
         return ti;
     };
     if (pair) asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
-    //@T 3
     const uint16_t mc_mask = wk.share ? 3 : (uint16_t)(1u << (blockIdx.x & 1));
 
     // the control warpgroup hands registers to the two softmax warpgroups (one instruction per warpgroup)
@@ -459,7 +462,6 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
                     else tma_load_4d(dst, tm, fb, 0, ti.row, 0, wk.g, hint);
                 }
             }
-            //@T (jj < 6 ? 8 + jj : 63)
             if (is_v && (ti.valid & 15) != 0) {
                 mbar_wait_warp(lane, fb, round);  // this fill has landed (every lane observes it)
                 const int n_rows = ((ti.valid + 15) & ~15) - ti.valid;
@@ -625,7 +627,6 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
                 const int keys = min(kSubN, ti.valid - hf * kSubN);
                 const bool last = n == n_sub - 1;
                 mbar_wait(bar(kBarSFull + t), par);
-                //@T (n < 12 ? 32 + (n >> 2) * 5 : 63)
                 if (!warp_active) {  // a warp without rows only keeps the barrier phases in step
                     if (lane == 0) {
                         mbar_arrive(bar(kBarSFree + t));
@@ -643,7 +644,6 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(bar(kBarSFree + t));  // Q.K^T of sub-unit n+4 may overwrite S now
-                //@T (n < 12 ? 33 + (n >> 2) * 5 : 63)
                 if (ti.tree || keys < kSubN) {
                     // keys past the tile's end, and (tree tiles) keys that are not ancestors-or-self of this
                     // row's node: the sub-unit's 64 mask bits -> -inf
@@ -753,7 +753,6 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
         const int t_last = (n_sub - 1) & 3;
         mbar_wait_warp(lane, bar(kBarAllDone), 0);  // every MMA done: O is final, the rings are free
         if (pair) asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");  // (see the control warps)
-        //@T 56
         // every team's (reference, row sum) of the row through the free V ring, one barrier: the final reference
         // is the one of the last sub-unit's owner, each sum is brought to it
         float2* xp = reinterpret_cast<float2*>(smem_gen + kOffV);
@@ -769,7 +768,6 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
         }
         const float inv = l_tot > 0.f ? __fdividef(1.f, l_tot) : 0.f;  // l = 0: every key of the chunk masked, or no key at all
         const float lse_v = l_tot > 0.f ? m_fin * pl.sm_scale + __logf(l_tot) : -INFINITY;
-        //@T 57
         const bool direct = wk.n_chunks == 1;
         const bool row_ok = rl < wk.rows;
         const size_t prow0 = (size_t)wk.group * pl.grp_rows + (size_t)wk.chunk * kTileM;
@@ -859,7 +857,6 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
             const unsigned expected = (unsigned)wk.n_chunks;
             unsigned* cnt = a.counters + 2 * wk.group;  // [0] arrivals, [1] done
             named_bar_sync(10, 512);  // every thread's partial-state writes happen before the leader's (cumulative) release
-            //@T 58
             unsigned done_before = 0;
             if (pl.last_merges) {
                 if (warp == 0 && lane == 0) {
@@ -898,11 +895,9 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
                     xl[0] = __int_as_float(ok);
                 }
                 named_bar_sync(9, 512);
-                //@T 59
                 if (__float_as_int(xl[0]))
                     merge_rows(pl, a, dbg_rows, wk, wk.rows * wk.chunk / wk.n_chunks, wk.rows * (wk.chunk + 1) / wk.n_chunks,
                                warp, lane);
-                //@T 60
                 if (warp == 0 && lane == 0) {
                     if (done_before == expected - 1) {  // last CTA out: everybody is past the wait
                         cnt[0] = 0;
@@ -919,11 +914,9 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
     if (warp == 18) {
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(kTmemCols) : "memory");
     }
-    //@T 61
     // no CTA leaves while its peer may still signal its barriers (every thread of the pair arrived after its last
     // remote operation; by now the peer's arrivals are an epilogue old)
     if (pair) asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
-    //@T 62
 }
 
 // ---- host side ----------------------------------------------------------------------------------
