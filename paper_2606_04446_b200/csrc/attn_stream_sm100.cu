@@ -158,6 +158,12 @@ __device__ __forceinline__ uint4 ld_cg_u4(const __nv_bfloat16* p) {
     asm volatile("ld.global.cg.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
     return v;
 }
+// Row sums of the partial states: the workspace's O region is sized for fp32 rows (common.cuh), this kernel's bf16
+// rows fill its first half; the sums sit right behind them.
+__device__ __forceinline__ float* part_sum(const AttnPlan& pl, const AttnArgs& a) {
+    const size_t rows_all = (size_t)pl.B * pl.Hkv * pl.n_mt * pl.grp_rows;
+    return reinterpret_cast<float*>(a.part_o16 + rows_all * kD);
+}
 __device__ __forceinline__ float bf_lo(uint32_t w) { return __uint_as_float(w << 16); }
 __device__ __forceinline__ float bf_hi(uint32_t w) { return __uint_as_float(w & 0xFFFF0000u); }
 
@@ -184,31 +190,37 @@ __device__ __forceinline__ void merge_rows(const AttnPlan& pl, const AttnArgs& a
         const int r = r0 + (idx >> 4), cg = idx & 15;
         const float* lp = a.part_lse + grp0 + r;
         const __nv_bfloat16* op = a.part_o16 + (grp0 + r) * kD + cg * 8;
-        float lv[kSB];
+        const float* sp = part_sum(pl, a) + grp0 + r;
+        float mv[kSB], sv[kSB];
         uint4 v[kSB];
 #pragma unroll
-        for (int i = 0; i < kSB; ++i) lv[i] = i < nc ? ld_cg_f32(lp + (size_t)i * kTileM) : -INFINITY;
+        for (int i = 0; i < kSB; ++i) {
+            mv[i] = i < nc ? ld_cg_f32(lp + (size_t)i * kTileM) : 0.f;
+            sv[i] = i < nc ? ld_cg_f32(sp + (size_t)i * kTileM) : 0.f;
+        }
 #pragma unroll
         for (int i = 0; i < kSB; ++i)
             if (i < nc) v[i] = ld_cg_u4(op + (size_t)i * kTileM * kD);
-        float m = lv[0];
+        // O = sum_i 2^(m_i - M) O_i / sum_i 2^(m_i - M) l_i over the states that saw a key (l_i > 0)
+        float m = -INFINITY;
 #pragma unroll
-        for (int i = 1; i < kSB; ++i) m = fmaxf(m, lv[i]);
+        for (int i = 0; i < kSB; ++i) m = sv[i] > 0.f ? fmaxf(m, mv[i]) : m;
 #pragma unroll 1
-        for (int i = kSB; i < nc; ++i) m = fmaxf(m, ld_cg_f32(lp + (size_t)i * kTileM));  // more than eight chunks
+        for (int i = kSB; i < nc; ++i)  // more than eight chunks
+            if (ld_cg_f32(sp + (size_t)i * kTileM) > 0.f) m = fmaxf(m, ld_cg_f32(lp + (size_t)i * kTileM));
         float ws = 0.f, wv[kSB];
 #pragma unroll
         for (int i = 0; i < kSB; ++i) {
-            wv[i] = lv[i] == -INFINITY ? 0.f : __expf(lv[i] - m);
-            ws += wv[i];
+            wv[i] = sv[i] > 0.f ? ex2(mv[i] - m) : 0.f;
+            ws += wv[i] * sv[i];
         }
 #pragma unroll 1
         for (int i = kSB; i < nc; ++i) {
-            const float l = ld_cg_f32(lp + (size_t)i * kTileM);
-            ws += l == -INFINITY ? 0.f : __expf(l - m);
+            const float l = ld_cg_f32(sp + (size_t)i * kTileM);
+            if (l > 0.f) ws += ex2(ld_cg_f32(lp + (size_t)i * kTileM) - m) * l;
         }
         const float inv = ws > 0.f ? __fdividef(1.f, ws) : 0.f;  // no key at all (L = 0, prefix-only mode): O = 0, LSE = -inf
-        const float lse = ws > 0.f ? m + __logf(ws) : -INFINITY;  // (1 <= ws <= 64: lg2.approx is accurate to ~1e-7 here)
+        const float lse = ws > 0.f ? (m + __log2f(ws)) * (1.f / kLog2e) : -INFINITY;
         float acc[8];
 #pragma unroll
         for (int c = 0; c < 8; ++c) acc[c] = 0.f;
@@ -223,8 +235,8 @@ __device__ __forceinline__ void merge_rows(const AttnPlan& pl, const AttnArgs& a
             }
 #pragma unroll 1
         for (int i = kSB; i < nc; ++i) {
-            const float l = ld_cg_f32(lp + (size_t)i * kTileM);
-            const float w1 = l == -INFINITY ? 0.f : __expf(l - m) * inv;
+            const float l = ld_cg_f32(sp + (size_t)i * kTileM);
+            const float w1 = l > 0.f ? ex2(ld_cg_f32(lp + (size_t)i * kTileM) - m) * inv : 0.f;
             const uint4 x = ld_cg_u4(op + (size_t)i * kTileM * kD);
             acc[0] += w1 * bf_lo(x.x); acc[1] += w1 * bf_hi(x.x);
             acc[2] += w1 * bf_lo(x.y); acc[3] += w1 * bf_hi(x.y);
@@ -753,10 +765,48 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
         const int t_last = (n_sub - 1) & 3;
         mbar_wait_warp(lane, bar(kBarAllDone), 0);  // every MMA done: O is final, the rings are free
         if (pair) asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");  // (see the control warps)
+        const bool direct = wk.n_chunks == 1;
+        const bool row_ok = rl < wk.rows;
+        const size_t prow0 = (size_t)wk.group * pl.grp_rows + (size_t)wk.chunk * kTileM;
+        float* xl = reinterpret_cast<float*>(smem_gen + kOffXL);  // (scratch word of the group wait below)
+        // per-warp staging: [32 rows][128 B] of fp32 (direct output) or [32 rows][64 B] of bf16 pairs (partial
+        // state), 16-byte chunks XOR-swizzled by the row
+        const uint32_t region = smem + kOffK + (uint32_t)warp * 4096u;
+        // A partial state leaves UNNORMALISED, relative to the row's final reference (which O in TMEM already is): its
+        // stores go out first and their way to L2 runs under the row-sum exchange below; the merge divides once.
+        if (!direct && warp_active) {
+            uint32_t ov[32];
+            tc_fence_after();
+            if (n_sub > 0) {
+                D2SD_TMEM_LD32(tmem + lane_addr + t * 32, ov, 0);
+                tmem_wait_ld();
+            }
+#pragma unroll
+            for (int c = 0; c < 32; c += 8) {  // 8 columns = one 16-byte chunk of bf16
+                const uint32_t chunk = (uint32_t)(c >> 3) ^ ((uint32_t)(lane >> 1) & 3u);
+                uint32_t pk[4];
+#pragma unroll
+                for (int e = 0; e < 4; ++e)
+                    pk[e] = n_sub > 0 ? pack2_bf16(__uint_as_float(ov[c + 2 * e]), __uint_as_float(ov[c + 2 * e + 1])) : 0u;
+                asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(region + (uint32_t)lane * 64u + chunk * 16u),
+                             "r"(pk[0]), "r"(pk[1]), "r"(pk[2]), "r"(pk[3])
+                             : "memory");
+            }
+            __syncwarp();
+#pragma unroll 1
+            for (int it = 0; it < 4; ++it) {
+                const int row = it * 8 + (lane >> 2), ck = lane & 3;
+                uint4 v;
+                asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];"
+                             : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w)
+                             : "r"(region + (uint32_t)row * 64u + (uint32_t)((ck ^ ((row >> 1) & 3)) * 16)));
+                const int r = w * 32 + row;  // row of the tile
+                if (r < wk.rows) *reinterpret_cast<uint4*>(a.part_o16 + (prow0 + r) * kD + t * 32 + ck * 8) = v;
+            }
+        }
         // every team's (reference, row sum) of the row through the free V ring, one barrier: the final reference
         // is the one of the last sub-unit's owner, each sum is brought to it
         float2* xp = reinterpret_cast<float2*>(smem_gen + kOffV);
-        float* xl = reinterpret_cast<float*>(smem_gen + kOffXL);  // (scratch word of the group wait below)
         xp[t * kTileM + rl] = make_float2(m_mine, l_mine);
         named_bar_sync(9, 512);
         const float m_fin = n_sub > 0 ? xp[t_last * kTileM + rl].x : -INFINITY;
@@ -766,15 +816,16 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
             const float2 ml = xp[tt * kTileM + rl];
             l_tot += ml.x == -INFINITY ? 0.f : ml.y * (ml.x == m_fin ? 1.f : ex2((ml.x - m_fin) * c2));
         }
-        const float inv = l_tot > 0.f ? __fdividef(1.f, l_tot) : 0.f;  // l = 0: every key of the chunk masked, or no key at all
-        const float lse_v = l_tot > 0.f ? m_fin * pl.sm_scale + __logf(l_tot) : -INFINITY;
-        const bool direct = wk.n_chunks == 1;
-        const bool row_ok = rl < wk.rows;
-        const size_t prow0 = (size_t)wk.group * pl.grp_rows + (size_t)wk.chunk * kTileM;
-        if (warp_active) {
-            // per-warp staging: [32 rows][128 B] of fp32 (direct output) or [32 rows][64 B] of bf16 pairs (partial
-            // state), 16-byte chunks XOR-swizzled by the row
-            const uint32_t region = smem + kOffK + (uint32_t)warp * 4096u;
+        if (!direct) {
+            // the row's state scalars: reference in log2 units and row sum (l = 0: every key of the chunk masked, or no
+            // key at all: the state carries no weight)
+            if (t == 0 && row_ok) {
+                a.part_lse[prow0 + rl] = l_tot > 0.f ? m_fin * c2 : 0.f;
+                part_sum(pl, a)[prow0 + rl] = l_tot;
+            }
+        } else if (warp_active) {
+            const float inv = l_tot > 0.f ? __fdividef(1.f, l_tot) : 0.f;
+            const float lse_v = l_tot > 0.f ? m_fin * pl.sm_scale + __logf(l_tot) : -INFINITY;
             const int G = pl.G;
             uint32_t ov[32];
             tc_fence_after();
@@ -784,69 +835,41 @@ attn_stream_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
             }
 #pragma unroll
             for (int c = 0; c < 32; ++c) ov[c] = n_sub > 0 ? __float_as_uint(__uint_as_float(ov[c]) * inv) : 0u;
-            if (direct) {
 #pragma unroll
-                for (int c = 0; c < 32; c += 4) {
-                    const uint32_t chunk = (uint32_t)(c >> 2) ^ ((uint32_t)lane & 7u);
-                    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(region + (uint32_t)lane * 128u + chunk * 16u),
-                                 "r"(ov[c]), "r"(ov[c + 1]), "r"(ov[c + 2]), "r"(ov[c + 3])
-                                 : "memory");
-                }
-                __syncwarp();
+            for (int c = 0; c < 32; c += 4) {
+                const uint32_t chunk = (uint32_t)(c >> 2) ^ ((uint32_t)lane & 7u);
+                asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(region + (uint32_t)lane * 128u + chunk * 16u),
+                             "r"(ov[c]), "r"(ov[c + 1]), "r"(ov[c + 2]), "r"(ov[c + 3])
+                             : "memory");
+            }
+            __syncwarp();
 #pragma unroll 1
-                for (int it = 0; it < 8; ++it) {
-                    const int row = it * 4 + (lane >> 3), ck = lane & 7;
-                    float4 v;
-                    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];"
-                                 : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
-                                 : "r"(region + (uint32_t)row * 128u + (uint32_t)((ck ^ (row & 7)) * 16)));
-                    const int r = w * 32 + row;  // row of the tile
-                    if (r >= wk.rows) continue;
-                    const int col = t * 32 + ck * 4;
-                    const int ra = wk.row_base + r, tn = ra / G;
-                    const size_t orow = ((size_t)wk.b * pl.T_cap + tn) * pl.Hq + wk.g * G + (ra - tn * G);
-                    if (dbg_rows) {
-                        float* d0 = dbg_rows + orow * (kD + 1) + col;
-                        d0[0] = v.x; d0[1] = v.y; d0[2] = v.z; d0[3] = v.w;
-                    } else {
-                        uint2 pk;
-                        pk.x = pack2_bf16(v.x, v.y);
-                        pk.y = pack2_bf16(v.z, v.w);
-                        *reinterpret_cast<uint2*>(a.out + orow * kD + col) = pk;
-                    }
-                }
-            } else {
-#pragma unroll
-                for (int c = 0; c < 32; c += 8) {  // 8 columns = one 16-byte chunk of bf16
-                    const uint32_t chunk = (uint32_t)(c >> 3) ^ ((uint32_t)(lane >> 1) & 3u);
-                    uint32_t pk[4];
-#pragma unroll
-                    for (int e = 0; e < 4; ++e) pk[e] = pack2_bf16(__uint_as_float(ov[c + 2 * e]), __uint_as_float(ov[c + 2 * e + 1]));
-                    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(region + (uint32_t)lane * 64u + chunk * 16u),
-                                 "r"(pk[0]), "r"(pk[1]), "r"(pk[2]), "r"(pk[3])
-                                 : "memory");
-                }
-                __syncwarp();
-#pragma unroll 1
-                for (int it = 0; it < 4; ++it) {
-                    const int row = it * 8 + (lane >> 2), ck = lane & 3;
-                    uint4 v;
-                    asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];"
-                                 : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w)
-                                 : "r"(region + (uint32_t)row * 64u + (uint32_t)((ck ^ ((row >> 1) & 3)) * 16)));
-                    const int r = w * 32 + row;  // row of the tile
-                    if (r < wk.rows) *reinterpret_cast<uint4*>(a.part_o16 + (prow0 + r) * kD + t * 32 + ck * 8) = v;
+            for (int it = 0; it < 8; ++it) {
+                const int row = it * 4 + (lane >> 3), ck = lane & 7;
+                float4 v;
+                asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];"
+                             : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
+                             : "r"(region + (uint32_t)row * 128u + (uint32_t)((ck ^ (row & 7)) * 16)));
+                const int r = w * 32 + row;  // row of the tile
+                if (r >= wk.rows) continue;
+                const int col = t * 32 + ck * 4;
+                const int ra = wk.row_base + r, tn = ra / G;
+                const size_t orow = ((size_t)wk.b * pl.T_cap + tn) * pl.Hq + wk.g * G + (ra - tn * G);
+                if (dbg_rows) {
+                    float* d0 = dbg_rows + orow * (kD + 1) + col;
+                    d0[0] = v.x; d0[1] = v.y; d0[2] = v.z; d0[3] = v.w;
+                } else {
+                    uint2 pk;
+                    pk.x = pack2_bf16(v.x, v.y);
+                    pk.y = pack2_bf16(v.z, v.w);
+                    *reinterpret_cast<uint2*>(a.out + orow * kD + col) = pk;
                 }
             }
             if (t == 0 && row_ok) {
-                if (!direct) {
-                    a.part_lse[prow0 + rl] = lse_v;
-                } else {
-                    const int ra = wk.row_base + rl, tn = ra / G;
-                    const size_t orow = ((size_t)wk.b * pl.T_cap + tn) * pl.Hq + wk.g * G + (ra - tn * G);
-                    if (dbg_rows) dbg_rows[orow * (kD + 1) + kD] = lse_v;
-                    else if (a.lse) a.lse[orow] = lse_v;
-                }
+                const int ra = wk.row_base + rl, tn = ra / G;
+                const size_t orow = ((size_t)wk.b * pl.T_cap + tn) * pl.Hq + wk.g * G + (ra - tn * G);
+                if (dbg_rows) dbg_rows[orow * (kD + 1) + kD] = lse_v;
+                else if (a.lse) a.lse[orow] = lse_v;
             }
         }
         if (!direct) {

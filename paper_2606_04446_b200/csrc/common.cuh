@@ -108,8 +108,11 @@ int32_t launch_commit_kv(const CommitArgs& a, cudaStream_t s);
 //    0..num_splits-1 are the prefix chunks, slot num_splits is the tree pass.
 //  tcgen05 kernels (attn_stream_sm100.cu, attn_duo_sm100.cu): a fixed 1 MiB header of self-resetting group
 //    counters (zero between calls) and the error word, then partials per group (request, kv head, M tile or
-//    item): O bf16 [group][grp_rows][d] and LSE fp32 [group][grp_rows]; chunk c of a group holds its rows at
+//    item): O bf16 [group][grp_rows][d] and one fp32 [group][grp_rows]; chunk c of a group holds its rows at
 //    c*128.. (one tile per CTA) or c*256.. (two tiles per CTA); the tree keys are key tiles of the same kernel.
+//    Two tiles per CTA: O normalised, the fp32 is the row's LSE.  One tile per CTA: O UNNORMALISED relative to the
+//    row's final reference maximum, the fp32 is that reference in log2 units, and the row sums (fp32
+//    [group][grp_rows]) sit behind the bf16 rows inside the O region (which is sized for fp32 rows).
 struct AttnPlan {
     int B, T_cap, W, Hq, Hkv, G, d;
     float sm_scale;
