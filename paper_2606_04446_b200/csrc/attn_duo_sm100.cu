@@ -385,7 +385,6 @@ attn_duo_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
             const int jr0 = wk.np - 1 - wk.j_begin, jr1 = wk.np + wk.nt - 1 - wk.j_begin;
             const int v0 = wk.L - (wk.np - 1) * kTileN, v1 = wk.T - (wk.nt - 1) * kTileN;
             auto valid_of = [&](int jj) { return jj == jr0 ? v0 : (jj == jr1 ? v1 : kTileN); };
-            auto keys_of = [&](int jj, int hf) { return max(0, min(kSubN, valid_of(jj) - hf * kSubN)); };
             if (warp == 18) {
                 for (int m = 0; m < n_m; ++m) mbar_wait(bar(kBarQFull + m), 0);  // (also with N = 0: no load left in flight)
                 uint32_t n = 0, ki = 0, kph = 0;
