@@ -194,6 +194,38 @@ def _attn_full_case(d2sd, oracle, cfg, q_scale=1.0, layer=0, pool_nan=False, ram
     return o, lse
 
 
+def test_attn_lengths_rewritten_by_preceding_kernel(d2sd, oracle):
+    """The one-tile kernel aims an L2 prefetch hint with the request lengths as they stand BEFORE the grid dependency
+    resolves.  Here the kernel right before each call is the one that rewrites ctx_len (a device copy on the same
+    stream), so the hint may see either value; every result must still be the oracle's for the lengths in force."""
+    cfg = synth.custom(61, B=1, gamma=16, K=4, V=64, ctx=(3000, 3000))
+    st = synth.make_step_inputs(cfg)
+    _, _, tree = oracle_tree(oracle, cfg, st)
+    ti = synth.make_tree_inputs(cfg, 0)
+    kv = synth.make_kv_cache(cfg, st["ctx_len"], 0)
+    q, k, v = bf16_cuda(ti["q"]), bf16_cuda(kv["k_cache"]), bf16_cuda(kv["v_cache"])
+    tk, tv = bf16_cuda(ti["tree_k"]), bf16_cuda(ti["tree_v"])
+    mask, tlen = mask_cuda(tree["mask"]), i32_cuda(tree["tree_len"])
+    L_full = int(st["ctx_len"][0])
+    lens = [L_full, 129, 2050, 0, L_full, 700]
+    srcs = [i32_cuda(np.array([L], np.int32)) for L in lens]
+    ctx = torch.zeros(1, dtype=torch.int32, device="cuda")
+    ws = d2sd.cascade_workspace(cfg.B, cfg.T_cap, ti["q"].shape[2], kv["k_cache"].shape[1], ti["q"].shape[3], L_full,
+                                device="cuda", kv_rows=kv["k_cache"].shape[0])
+    outs = []
+    for src in srcs:  # all enqueued back to back: copy (writes ctx_len), attention, copy, attention, ...
+        ctx.copy_(src)
+        o, lse = d2sd.cascade_verify_attn(q, k, v, None, None, ctx, tk, tv, mask, tlen, L_full, workspace=ws)
+        outs.append((o.clone(), lse.clone()))
+    torch.cuda.synchronize()
+    vr = valid_rows(tree["tree_len"], cfg.T_cap)
+    for L, (o, lse) in zip(lens, outs):
+        ro, rl = oracle.attention(ti["q"], kv["k_cache"], kv["v_cache"], kv["kv_indptr"], kv["kv_indices"],
+                                  kv["page_size"], np.array([L], np.int32), ti["tree_k"], ti["tree_v"], tree["mask"],
+                                  tree["tree_len"], which="full")
+        check_rows(o.float().cpu().numpy()[vr], lse.cpu().numpy()[vr], ro[vr], rl[vr], f"ctx_len rewritten to {L}")
+
+
 @pytest.mark.parametrize("impl", IMPLS)
 def test_attn_config1_full(d2sd, oracle, impl):
     _attn_full_case(d2sd, oracle, synth.CONFIGS[1], impl=impl)
