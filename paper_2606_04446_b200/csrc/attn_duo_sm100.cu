@@ -258,6 +258,19 @@ attn_duo_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant_
         const int G = pl.G;
         wk.g = blockIdx.y;
         wk.b = blockIdx.z;
+        if (pl.last_merges && pl.B <= 32) {
+            // Several waves: blocks are handed out in grid order, so the requests are taken longest first (slice z of
+            // the grid serves the request of rank z by context length, ties by index) and the last, partly filled
+            // wave is made of short CTAs.  Every warp computes the same permutation.
+            const int Lz = lane < pl.B ? a.ctx_len[lane] : -1;
+            int rank = 0;
+            for (int j = 0; j < pl.B; ++j) {
+                const int Lj = __shfl_sync(0xffffffffu, Lz, j);
+                rank += (Lj > Lz || (Lj == Lz && j < lane)) ? 1 : 0;
+            }
+            const unsigned hit = __ballot_sync(0xffffffffu, lane < pl.B && rank == (int)blockIdx.z);
+            wk.b = __ffs(hit) - 1;
+        }
         int x = blockIdx.x, n_static;
         bool duo;
         if (x < pl.n_pair * pl.chunks_a) {
